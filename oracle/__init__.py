@@ -1,0 +1,252 @@
+"""ctypes loader for the CPU oracle (oracle/feds_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+`--impl reference` arm import this. Argument marshalling only; all arithmetic is in the C file, which
+cites the paper passage each function follows. Format constants (G, F, LEAF) are DESIGN.md section 2's.
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+G_BLOCKS = 8      # blocks per DCT-path leaf
+FANOUT = 16       # children per Merkle node
+LEAF_BYTES = 2048  # bytes per DWT-path leaf
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+    return _lib
+
+
+def _u8(a):
+    a = np.ascontiguousarray(a, dtype=np.uint8)
+    return a, a.ctypes.data_as(C.POINTER(C.c_uint8))
+
+
+def _key(b):
+    b = bytes(b)
+    assert len(b) == 16
+    return (C.c_uint8 * 16).from_buffer_copy(b)
+
+
+def sha256(msg) -> bytes:
+    a, p = _u8(np.frombuffer(bytes(msg), dtype=np.uint8) if not isinstance(msg, np.ndarray) else msg)
+    out = (C.c_uint8 * 32)()
+    lib().orc_sha256(p, C.c_uint64(a.size), out)
+    return bytes(out)
+
+
+def merkle_root(digests: bytes, fanout: int = FANOUT) -> bytes:
+    a, p = _u8(np.frombuffer(bytes(digests), dtype=np.uint8))
+    assert a.size % 32 == 0
+    out = (C.c_uint8 * 32)()
+    rc = lib().orc_merkle_root(p, C.c_uint64(a.size // 32), C.c_int(fanout), out)
+    assert rc == 0, rc
+    return bytes(out)
+
+
+def merkle_stream(data, leaf_bytes: int = LEAF_BYTES, fanout: int = FANOUT) -> bytes:
+    a, p = _u8(data if isinstance(data, np.ndarray) else np.frombuffer(bytes(data), dtype=np.uint8))
+    out = (C.c_uint8 * 32)()
+    rc = lib().orc_merkle_stream(p, C.c_uint64(a.size), C.c_uint64(leaf_bytes), C.c_int(fanout), out)
+    assert rc == 0, rc
+    return bytes(out)
+
+
+def merkle_blocks(data, n_rows: int, nbc: int, per_block: int, g: int = G_BLOCKS, fanout: int = FANOUT) -> bytes:
+    a, p = _u8(data if isinstance(data, np.ndarray) else np.frombuffer(bytes(data), dtype=np.uint8))
+    assert a.size == n_rows * nbc * per_block
+    out = (C.c_uint8 * 32)()
+    rc = lib().orc_merkle_blocks(p, C.c_uint64(n_rows), C.c_uint64(nbc), C.c_uint64(per_block), C.c_int(g),
+                                 C.c_int(fanout), out)
+    assert rc == 0, rc
+    return bytes(out)
+
+
+def aes_sbox() -> bytes:
+    out = (C.c_uint8 * 256)()
+    lib().orc_aes_sbox(out)
+    return bytes(out)
+
+
+def aes128_expand_key(key) -> bytes:
+    rk = (C.c_uint8 * 176)()
+    lib().orc_aes128_expand_key(_key(key), rk)
+    return bytes(rk)
+
+
+def aes128_encrypt_block(key, block) -> bytes:
+    rk = (C.c_uint8 * 176).from_buffer_copy(aes128_expand_key(key))
+    out = (C.c_uint8 * 16)()
+    lib().orc_aes128_encrypt_block(rk, _key(block), out)
+    return bytes(out)
+
+
+def aes128_ctr_xor(key, nonce, data, first_block: int = 0) -> bytes:
+    a = np.array(np.frombuffer(bytes(data), dtype=np.uint8))  # writable copy
+    p = a.ctypes.data_as(C.POINTER(C.c_uint8))
+    lib().orc_aes128_ctr_xor(_key(key), _key(nonce), C.c_uint64(first_block), p, C.c_uint64(a.size))
+    return a.tobytes()
+
+
+def dct8x8(x) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.float64).reshape(64)
+    out = np.empty(64, dtype=np.float64)
+    lib().orc_dct8x8(x.ctypes.data_as(C.POINTER(C.c_double)), out.ctypes.data_as(C.POINTER(C.c_double)))
+    return out.reshape(8, 8)
+
+
+def idct8x8(X) -> np.ndarray:
+    X = np.ascontiguousarray(X, dtype=np.float64).reshape(64)
+    out = np.empty(64, dtype=np.float64)
+    lib().orc_idct8x8(X.ctypes.data_as(C.POINTER(C.c_double)), out.ctypes.data_as(C.POINTER(C.c_double)))
+    return out.reshape(8, 8)
+
+
+def zigzag(z: int):
+    r, q = C.c_int(), C.c_int()
+    rc = lib().orc_zigzag(C.c_int(z), C.byref(r), C.byref(q))
+    assert rc == 0
+    return r.value, q.value
+
+
+def _img(image):
+    image = np.ascontiguousarray(image, dtype=np.uint8)
+    if image.ndim == 2:
+        image = image[:, :, None]
+    h, w, c = image.shape
+    return image, h, w, c
+
+
+def dct_private_bytes(w, h, c, k):
+    return (w // 8) * (h // 8) * c * (k + 1) * 4
+
+
+def dct_public_bytes(w, h, c, k):
+    return (w // 8) * (h // 8) * c * (63 - k) * 4
+
+
+def dwt_private_bytes(w, h, c, levels):
+    return (w >> levels) * (h >> levels) * c * 2
+
+
+def dwt_public_bytes(w, h, c, levels):
+    return (w * h - (w >> levels) * (h >> levels)) * c * 2
+
+
+def dct_coefficients(image) -> np.ndarray:
+    """double coefficients [C*nbr*nbc][64] in zigzag order (fragment block order)."""
+    image, h, w, c = _img(image)
+    nb = c * (h // 8) * (w // 8)
+    out = np.empty((nb, 64), dtype=np.float64)
+    rc = lib().orc_dct_coefficients(image.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c,
+                                    out.ctypes.data_as(C.POINTER(C.c_double)))
+    assert rc == 0, rc
+    return out
+
+
+def fragment_from_coef32(coef32, w, h, c, k, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    coef32 = np.ascontiguousarray(coef32, dtype=np.float32)
+    assert coef32.size == 64 * c * (h // 8) * (w // 8)
+    priv = np.empty(dct_private_bytes(w, h, c, k), dtype=np.uint8)
+    pub = np.empty(dct_public_bytes(w, h, c, k), dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_from_coef32(coef32.ctypes.data_as(C.POINTER(C.c_float)), w, h, c, k, _key(key), _key(nonce),
+                                        g, fanout, priv.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                        pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    assert rc == 0, rc
+    return priv, pub, bytes(dg)
+
+
+def fragment_dct(image, k, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    image, h, w, c = _img(image)
+    priv = np.empty(dct_private_bytes(w, h, c, k), dtype=np.uint8)
+    pub = np.empty(dct_public_bytes(w, h, c, k), dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_dct(image.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c, k, _key(key), _key(nonce), g, fanout,
+                                priv.ctypes.data_as(C.POINTER(C.c_uint8)), pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    if rc != 0:
+        raise ValueError("orc_fragment_dct rc=%d" % rc)
+    return priv, pub, bytes(dg)
+
+
+def defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=None, g=G_BLOCKS, fanout=FANOUT):
+    priv, pp = _u8(priv)
+    pub, qq = _u8(pub)
+    assert priv.size == dct_private_bytes(w, h, c, k) and pub.size == dct_public_bytes(w, h, c, k)
+    out = np.empty((h, w, c), dtype=np.uint8)
+    flags = C.c_uint32(0)
+    exp = (C.c_uint8 * 64).from_buffer_copy(bytes(expected)) if expected is not None else None
+    rc = lib().orc_defragment_dct(pp, qq, w, h, c, k, _key(key), _key(nonce), g, fanout, exp,
+                                  out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(flags))
+    if rc != 0:
+        raise ValueError("orc_defragment_dct rc=%d" % rc)
+    return out, flags.value
+
+
+def dwt53_fwd_1d(x) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    y = np.empty_like(x)
+    lib().orc_dwt53_fwd_1d(x.ctypes.data_as(C.POINTER(C.c_int32)), C.c_int(x.size), y.ctypes.data_as(C.POINTER(C.c_int32)))
+    return y
+
+
+def dwt53_inv_1d(y) -> np.ndarray:
+    y = np.ascontiguousarray(y, dtype=np.int32)
+    x = np.empty_like(y)
+    lib().orc_dwt53_inv_1d(y.ctypes.data_as(C.POINTER(C.c_int32)), C.c_int(y.size), x.ctypes.data_as(C.POINTER(C.c_int32)))
+    return x
+
+
+def dwt_coefficients(image, levels) -> np.ndarray:
+    """int32 [C][H][W] Mallat-layout planes of the L-level transform of (pixel - 128)."""
+    image, h, w, c = _img(image)
+    out = np.empty((c, h, w), dtype=np.int32)
+    rc = lib().orc_dwt_coefficients(image.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c, levels,
+                                    out.ctypes.data_as(C.POINTER(C.c_int32)))
+    if rc != 0:
+        raise ValueError("orc_dwt_coefficients rc=%d" % rc)
+    return out
+
+
+def dwt_inverse_plane(plane, levels) -> np.ndarray:
+    p = np.array(plane, dtype=np.int32, order="C")
+    h, w = p.shape
+    rc = lib().orc_dwt53_inv_plane(p.ctypes.data_as(C.POINTER(C.c_int32)), w, h, levels)
+    assert rc == 0
+    return p
+
+
+def fragment_dwt(image, levels, key, nonce, leaf_bytes=LEAF_BYTES, fanout=FANOUT):
+    image, h, w, c = _img(image)
+    if w <= 0 or h <= 0 or levels < 1 or levels > 6 or w % (1 << levels) or h % (1 << levels):
+        raise ValueError("bad DWT dims")
+    priv = np.empty(dwt_private_bytes(w, h, c, levels), dtype=np.uint8)
+    pub = np.empty(dwt_public_bytes(w, h, c, levels), dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_dwt(image.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c, levels, _key(key), _key(nonce),
+                                C.c_uint64(leaf_bytes), fanout, priv.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    if rc != 0:
+        raise ValueError("orc_fragment_dwt rc=%d" % rc)
+    return priv, pub, bytes(dg)
+
+
+def defragment_dwt(priv, pub, w, h, c, levels, key, nonce, expected=None, leaf_bytes=LEAF_BYTES, fanout=FANOUT):
+    priv, pp = _u8(priv)
+    pub, qq = _u8(pub)
+    assert priv.size == dwt_private_bytes(w, h, c, levels) and pub.size == dwt_public_bytes(w, h, c, levels)
+    out = np.empty((h, w, c), dtype=np.uint8)
+    flags = C.c_uint32(0)
+    exp = (C.c_uint8 * 64).from_buffer_copy(bytes(expected)) if expected is not None else None
+    rc = lib().orc_defragment_dwt(pp, qq, w, h, c, levels, _key(key), _key(nonce), C.c_uint64(leaf_bytes), fanout, exp,
+                                  out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(flags))
+    if rc != 0:
+        raise ValueError("orc_defragment_dwt rc=%d" % rc)
+    return out, flags.value
