@@ -1,0 +1,156 @@
+/*
+ * feds.h — C ABI of libfeds: selective-encryption fragmentation of 8-bit images on one B200 (sm_100a).
+ *
+ * Method: arXiv 1512.02951 section 6 ("P:n" = PAPER.md line n); byte format: DESIGN.md section 2.
+ *
+ * Conventions (all entry points)
+ *   - `d_*` pointers are DEVICE pointers, 16-byte aligned; `key`/`nonce` (16 bytes each) are HOST pointers and are
+ *     read before the call returns. `h_*` pointers (host-staged entry points only) are HOST pointers.
+ *   - The caller owns every buffer. The library allocates nothing, keeps no global state, logs nothing.
+ *   - All work is enqueued on `stream`; no call synchronises the device. Argument errors are returned before
+ *     anything is enqueued; a failed launch returns FEDS_ERR_CUDA (see feds_last_cuda_error); asynchronous faults
+ *     surface at the caller's next synchronisation, as with any CUDA library.
+ *   - Input, fragments, workspace and output must not alias.
+ *   - Image layout: uint8[H][W][C], interleaved, tight pitch, C in {1,3,4}; the transform runs per channel plane.
+ *   - There is no CPU fallback anywhere in this library.
+ */
+#ifndef FEDS_H
+#define FEDS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__CUDACC__) || defined(__CUDA_RUNTIME_API_H__) || defined(__DRIVER_TYPES_H__)
+#include <cuda_runtime_api.h>
+typedef cudaStream_t feds_stream_t;
+#else
+typedef struct CUstream_st *feds_stream_t; /* identical to cudaStream_t */
+#endif
+
+typedef enum {
+    FEDS_OK = 0,
+    FEDS_ERR_NULL_POINTER = 1,
+    FEDS_ERR_BAD_DIMS = 2,            /* w,h <= 0; not a multiple of 8 (DCT) / of 2^levels (DWT) */
+    FEDS_ERR_BAD_PARAM = 3,           /* k not in [0,63]; levels not in [1,6]; channels not in {1,3,4}; n_images < 1; bad stride/flags */
+    FEDS_ERR_WORKSPACE_TOO_SMALL = 4,
+    FEDS_ERR_CUDA = 5,                /* a launch or copy failed; cudaError_t kept for feds_last_cuda_error() */
+    FEDS_ERR_MISALIGNED = 6           /* a device pointer or stride is not 16-byte aligned */
+} feds_status;
+
+/* Flags for the *_batch entry points. */
+#define FEDS_FLAG_NONE 0u
+#define FEDS_FLAG_NO_DIGEST 1u /* skip step 5 (SHA-256 Merkle digests); d_digests is not written. Measurement of the HBM-bound core. */
+
+const char *feds_status_string(feds_status s);
+int feds_last_cuda_error(void); /* cudaError_t of the most recent FEDS_ERR_CUDA on this thread, else 0 */
+
+/* Frozen format constants: blocks per DCT leaf G, Merkle fan-out F, bytes per DWT leaf. */
+void feds_merkle_params(int *g_blocks, int *fanout, int *dwt_leaf_bytes);
+
+/* Fragment sizes in bytes for ONE image (DC + first k zigzag AC -> private; LL_L -> private).
+ * Return 0 for invalid arguments. */
+size_t feds_dct_private_bytes(int w, int h, int c, int k);       /* (w/8)(h/8) c (k+1) 4  */
+size_t feds_dct_public_bytes(int w, int h, int c, int k);        /* (w/8)(h/8) c (63-k) 4 */
+size_t feds_dwt_private_bytes(int w, int h, int c, int levels);  /* (w>>L)(h>>L) c 2      */
+size_t feds_dwt_public_bytes(int w, int h, int c, int levels);   /* (w h - (w>>L)(h>>L)) c 2 */
+/* Workspace bytes for ONE image (leaf digests + tree levels; DWT: also the intermediate LL planes).
+ * A batch of n images needs n times this. */
+size_t feds_workspace_bytes(int w, int h, int c, int k_or_levels, int is_dwt);
+
+/*
+ * feds_fragment_dct — steps 1-5 of the path (P:541-545 DCT 8x8, P:488-494 selection,
+ * P:607 + P:1018 AES-128-CTR on the private part, BASELINE north_star SHA-256 digests).
+ *   d_image    in : uint8[h][w][c]
+ *   k          in : number of AC coefficients (zigzag order) that join the DC in the private fragment, 0..63
+ *   key, nonce in : HOST, 16 bytes each; nonce = initial counter block T_0, T_i = (T_0 + i) mod 2^128 big-endian
+ *   d_private  out: feds_dct_private_bytes() bytes: float32 LE [block][z = 0..k], AES-128-CTR ciphertext
+ *   d_public   out: feds_dct_public_bytes() bytes: float32 LE [block][z = k+1..63], plaintext
+ *   d_digests  out: 64 bytes: Merkle root of the private fragment (as stored) || root of the public fragment
+ *   d_workspace   : >= feds_workspace_bytes(w,h,c,k,0) bytes of scratch
+ */
+feds_status feds_fragment_dct(const uint8_t *d_image, int w, int h, int c, int k, const uint8_t key[16],
+                              const uint8_t nonce[16], uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests,
+                              void *d_workspace, size_t workspace_bytes, feds_stream_t stream);
+
+/*
+ * feds_defragment_dct — steps 6-8 (decrypt, reassemble, inverse transform; round to nearest, clamp).
+ *   d_expected_digests in : 64 bytes or NULL. Non-NULL: the digests of the fragments as received are recomputed
+ *                           and compared; d_verify_flags[0] = bit0 (private mismatch) | bit1 (public mismatch).
+ *                           NULL: no verification, d_verify_flags is not written.
+ *   d_image_out       out: uint8[h][w][c]; written regardless of the verification result.
+ */
+feds_status feds_defragment_dct(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k,
+                                const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
+                                size_t workspace_bytes, feds_stream_t stream);
+
+/*
+ * feds_fragment_dwt / feds_defragment_dwt — rows D1-D8: level shift -128, `levels`-level whole-image
+ * Le Gall 5/3 integer lifting, rows then columns, LL_levels -> private under AES-128-CTR,
+ * the other subbands -> public (order: channel, level L..1, HL, LH, HH, row-major int16 LE), SHA-256 Merkle
+ * digests over 2048-byte leaves of each fragment stream; the inverse is exact.
+ */
+feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int levels, const uint8_t key[16],
+                              const uint8_t nonce[16], uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests,
+                              void *d_workspace, size_t workspace_bytes, feds_stream_t stream);
+
+feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,
+                                const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
+                                size_t workspace_bytes, feds_stream_t stream);
+
+/*
+ * Batched DCT entry points ("series of images"): n_images images of identical shape, image i at
+ * d_images + i*image_stride, fragments at d_private + i*private_stride / d_public + i*public_stride, digests at
+ * d_digests + 64 i, verify flags at d_verify_flags + i. Every image is an independent CTR message with its own
+ * nonce ("different IV for each input matrix"): d_nonces is a DEVICE array uint8[n_images][16].
+ * One launch per stage spans the whole batch. Strides are in bytes, multiples of 16, >= the per-image size.
+ * Workspace: n_images * feds_workspace_bytes(...).
+ */
+feds_status feds_fragment_dct_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c,
+                                    int k, const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private,
+                                    size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests,
+                                    void *d_workspace, size_t workspace_bytes, unsigned flags, feds_stream_t stream);
+
+feds_status feds_defragment_dct_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public,
+                                      size_t public_stride, int n_images, int w, int h, int c, int k,
+                                      const uint8_t key[16], const uint8_t *d_nonces,
+                                      const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                      uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                                      unsigned flags, feds_stream_t stream);
+
+/*
+ * Host-staged batch fragment (BASELINE north_star "stream-overlapped host<->device staging"; the paper's
+ * Fig. 11 overlay, moved to PCIe): images, fragments and digests live in HOST memory (pinned for
+ * the copies to overlap); the batch is cut into n_streams chunks-in-flight, each chunk doing H2D -> fragment
+ * -> D2H on its own stream. The caller supplies the streams and one device scratch area of
+ * feds_fragment_dct_host_scratch_bytes() bytes. h_nonces is uint8[n_images][16] on the HOST.
+ * Returns after enqueuing; synchronise the given streams before reading the outputs.
+ */
+size_t feds_fragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k);
+feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w, int h, int c, int k,
+                                   const uint8_t key[16], const uint8_t *h_nonces, uint8_t *h_private,
+                                   uint8_t *h_public, uint8_t *h_digests, int images_per_chunk, void *d_scratch,
+                                   size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags);
+
+/*
+ * Host-side arithmetic self-checks of the device building blocks (the same __host__ __device__ functions the
+ * kernels call), usable without a GPU. Not part of the data path.
+ *   feds_debug_sha256_host   : SHA-256 of a host buffer through the kernels' compression function.
+ *   feds_debug_aes128_host   : one AES-128 block through the kernels' T-table rounds.
+ *   feds_debug_dct8x8_host   : forward (inverse=0) / inverse (inverse=1) 8x8 float32 transform, row-major.
+ *   feds_debug_zigzag_host   : the kernels' zigzag table, out[z] = 8*row + col.
+ */
+void feds_debug_sha256_host(const uint8_t *msg, size_t n, uint8_t out[32]);
+void feds_debug_aes128_host(const uint8_t key[16], const uint8_t in[16], uint8_t out[16]);
+void feds_debug_dct8x8_host(const float in[64], float out[64], int inverse);
+void feds_debug_zigzag_host(int out[64]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FEDS_H */

@@ -1,0 +1,211 @@
+"""Thin ctypes binding over libfeds.so (include/feds.h): argument marshalling only.
+
+torch supplies device memory and streams; every step of the path runs in the library's CUDA kernels. There is no
+CPU fallback: if the library is missing or fails to load, importing this module raises.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfeds.so")
+
+FLAG_NONE = 0
+FLAG_NO_DIGEST = 1
+
+STATUS = {0: "FEDS_OK", 1: "FEDS_ERR_NULL_POINTER", 2: "FEDS_ERR_BAD_DIMS", 3: "FEDS_ERR_BAD_PARAM",
+          4: "FEDS_ERR_WORKSPACE_TOO_SMALL", 5: "FEDS_ERR_CUDA", 6: "FEDS_ERR_MISALIGNED"}
+
+# every symbol include/feds.h declares
+SYMBOLS = [
+    "feds_status_string", "feds_last_cuda_error", "feds_merkle_params",
+    "feds_dct_private_bytes", "feds_dct_public_bytes", "feds_dwt_private_bytes", "feds_dwt_public_bytes",
+    "feds_workspace_bytes",
+    "feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
+    "feds_fragment_dct_batch", "feds_defragment_dct_batch",
+    "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
+    "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
+]
+
+
+class FedsError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__("%s returned %s (%d)" % (where, STATUS.get(code, "?"), code))
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libfeds.so is not built: run `python -m paper_1512_02951_b200.build` (no CPU fallback exists)")
+    lib = C.CDLL(LIB_PATH)
+    vp, sz, i, u8p = C.c_void_p, C.c_size_t, C.c_int, C.c_char_p
+    lib.feds_status_string.restype = C.c_char_p
+    lib.feds_status_string.argtypes = [i]
+    lib.feds_last_cuda_error.restype = i
+    lib.feds_merkle_params.argtypes = [C.POINTER(i)] * 3
+    for name in ["feds_dct_private_bytes", "feds_dct_public_bytes", "feds_dwt_private_bytes", "feds_dwt_public_bytes"]:
+        getattr(lib, name).restype = sz
+        getattr(lib, name).argtypes = [i, i, i, i]
+    lib.feds_workspace_bytes.restype = sz
+    lib.feds_workspace_bytes.argtypes = [i, i, i, i, i]
+    lib.feds_fragment_dct.argtypes = [vp, i, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
+    lib.feds_fragment_dwt.argtypes = lib.feds_fragment_dct.argtypes
+    lib.feds_defragment_dct.argtypes = [vp, vp, i, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
+    lib.feds_defragment_dwt.argtypes = lib.feds_defragment_dct.argtypes
+    lib.feds_fragment_dct_batch.argtypes = [vp, i, sz, i, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, C.c_uint, vp]
+    lib.feds_defragment_dct_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, u8p, vp, vp, vp, sz, vp, vp, sz, C.c_uint, vp]
+    lib.feds_fragment_dct_host_scratch_bytes.restype = sz
+    lib.feds_fragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
+    lib.feds_fragment_dct_host.argtypes = [vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
+    lib.feds_debug_sha256_host.argtypes = [u8p, sz, vp]
+    lib.feds_debug_aes128_host.argtypes = [u8p, u8p, vp]
+    lib.feds_debug_dct8x8_host.argtypes = [vp, vp, i]
+    lib.feds_debug_zigzag_host.argtypes = [vp]
+    for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
+                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host"]:
+        getattr(lib, name).restype = i
+    return lib
+
+
+lib = _load()
+
+
+def _check(code, where):
+    if code != 0:
+        raise FedsError(code, where)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _stream(stream):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def merkle_params():
+    g, f, l = C.c_int(), C.c_int(), C.c_int()
+    lib.feds_merkle_params(C.byref(g), C.byref(f), C.byref(l))
+    return g.value, f.value, l.value
+
+
+def dct_private_bytes(w, h, c, k):
+    return lib.feds_dct_private_bytes(w, h, c, k)
+
+
+def dct_public_bytes(w, h, c, k):
+    return lib.feds_dct_public_bytes(w, h, c, k)
+
+
+def dwt_private_bytes(w, h, c, levels):
+    return lib.feds_dwt_private_bytes(w, h, c, levels)
+
+
+def dwt_public_bytes(w, h, c, levels):
+    return lib.feds_dwt_public_bytes(w, h, c, levels)
+
+
+def workspace_bytes(w, h, c, k_or_levels, is_dwt=False):
+    return lib.feds_workspace_bytes(w, h, c, k_or_levels, 1 if is_dwt else 0)
+
+
+def _u8(n, device):
+    return torch.empty(max(int(n), 16), dtype=torch.uint8, device=device)
+
+
+def _hwc(image):
+    assert image.dtype == torch.uint8 and image.is_cuda and image.is_contiguous()
+    if image.dim() == 2:
+        image = image.unsqueeze(-1)
+    h, w, c = image.shape
+    return image, int(w), int(h), int(c)
+
+
+def fragment_dct(image, k, key, nonce, stream=None, workspace=None):
+    """feds_fragment_dct: image uint8[H][W][C] (cuda) -> (private, public, digests[64]) device tensors."""
+    image, w, h, c = _hwc(image)
+    dev = image.device
+    priv = _u8(dct_private_bytes(w, h, c, k), dev)
+    pub = _u8(dct_public_bytes(w, h, c, k), dev)
+    dg = _u8(64, dev)
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _check(lib.feds_fragment_dct(_ptr(image), w, h, c, k, bytes(key), bytes(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
+                                 ws.numel(), _stream(stream)), "feds_fragment_dct")
+    return priv[:dct_private_bytes(w, h, c, k)], pub[:dct_public_bytes(w, h, c, k)], dg
+
+
+def defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=None, stream=None, workspace=None):
+    """feds_defragment_dct -> (image uint8[H][W][C], flags int32[1] or None)."""
+    dev = priv.device
+    out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
+    flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _check(lib.feds_defragment_dct(_ptr(priv), _ptr(pub), w, h, c, k, bytes(key), bytes(nonce), _ptr(expected), _ptr(out),
+                                   _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dct")
+    return out, flags
+
+
+def fragment_dwt(image, levels, key, nonce, stream=None, workspace=None):
+    image, w, h, c = _hwc(image)
+    dev = image.device
+    priv = _u8(dwt_private_bytes(w, h, c, levels), dev)
+    pub = _u8(dwt_public_bytes(w, h, c, levels), dev)
+    dg = _u8(64, dev)
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
+    _check(lib.feds_fragment_dwt(_ptr(image), w, h, c, levels, bytes(key), bytes(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
+                                 ws.numel(), _stream(stream)), "feds_fragment_dwt")
+    return priv[:dwt_private_bytes(w, h, c, levels)], pub[:dwt_public_bytes(w, h, c, levels)], dg
+
+
+def defragment_dwt(priv, pub, w, h, c, levels, key, nonce, expected=None, stream=None, workspace=None):
+    dev = priv.device
+    out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
+    flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
+    _check(lib.feds_defragment_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, bytes(key), bytes(nonce), _ptr(expected), _ptr(out),
+                                   _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dwt")
+    return out, flags
+
+
+class DctBatch:
+    """Pre-allocated buffers for feds_fragment_dct_batch / feds_defragment_dct_batch on n images of one shape."""
+
+    def __init__(self, n, w, h, c, k, device="cuda"):
+        self.n, self.w, self.h, self.c, self.k = n, w, h, c, k
+        self.image_bytes = w * h * c
+        self.priv_bytes = dct_private_bytes(w, h, c, k)
+        self.pub_bytes = dct_public_bytes(w, h, c, k)
+        self.priv = _u8(n * self.priv_bytes, device)
+        self.pub = _u8(n * self.pub_bytes, device)
+        self.digests = _u8(n * 64, device)
+        self.ws = _u8(n * workspace_bytes(w, h, c, k), device)
+        self.flags_out = torch.zeros(n, dtype=torch.int32, device=device)
+
+    def fragment(self, images, key, d_nonces, flags=FLAG_NONE, stream=None):
+        assert images.is_cuda and images.dtype == torch.uint8 and images.is_contiguous() and images.numel() == self.n * self.image_bytes
+        _check(lib.feds_fragment_dct_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, self.k, bytes(key),
+                                           _ptr(d_nonces), _ptr(self.priv), self.priv_bytes, _ptr(self.pub), self.pub_bytes,
+                                           _ptr(self.digests), _ptr(self.ws), self.ws.numel(), flags, _stream(stream)),
+               "feds_fragment_dct_batch")
+
+    def defragment(self, images_out, key, d_nonces, expected=None, flags=FLAG_NONE, stream=None):
+        _check(lib.feds_defragment_dct_batch(_ptr(self.priv), self.priv_bytes, _ptr(self.pub), self.pub_bytes, self.n, self.w, self.h,
+                                             self.c, self.k, bytes(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
+                                             self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
+                                             _stream(stream)), "feds_defragment_dct_batch")
+
+
+def fragment_dct_host(h_images, w, h, c, k, key, h_nonces, h_priv, h_pub, h_digests, images_per_chunk, d_scratch, streams,
+                      flags=FLAG_NONE):
+    """feds_fragment_dct_host: pinned host tensors in/out, staged over `streams` (torch.cuda.Stream list)."""
+    n = h_images.numel() // (w * h * c)
+    arr = (C.c_void_p * len(streams))(*[s.cuda_stream for s in streams])
+    _check(lib.feds_fragment_dct_host(_ptr(h_images), n, w, h, c, k, bytes(key), _ptr(h_nonces), _ptr(h_priv), _ptr(h_pub),
+                                      _ptr(h_digests), images_per_chunk, _ptr(d_scratch), d_scratch.numel(), arr, len(streams), flags),
+           "feds_fragment_dct_host")
+
+
+def host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k):
+    return lib.feds_fragment_dct_host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k)

@@ -1,0 +1,189 @@
+// feds_hash.cuh — stream-level kernels shared by both transform paths: SHA-256 over fixed-size leaves of a byte
+// stream (DWT path), the upper Merkle levels (2.1), AES-128-CTR over a byte stream, digest compare.
+#pragma once
+#include "feds_device.cuh"
+#include "feds_dct.cuh"  // g_aes, load_aes_tables, store_digest
+
+namespace feds {
+
+constexpr int HASH_THREADS = 128;
+
+// ------------------------------------------------------------------------------------------------------------
+// Upper Merkle levels: node j of tree t = SHA-256(children [j*F, min((j+1)*F, n_in)) concatenated), 32 B each.
+// Trees are (image, fragment) pairs laid out [tree][n][32]; the last level writes straight into the digest buffer.
+// ------------------------------------------------------------------------------------------------------------
+struct MerkleLevelParams {
+    const uint8_t *in;
+    uint8_t *out;
+    unsigned n_in, n_out;       // per tree
+    unsigned n_trees;
+    size_t in_tree_stride, out_tree_stride;  // bytes
+    int odd_trees_only_if_nonempty;  // 1: skip odd trees (public fragments) because they are empty (k = 63)
+};
+
+__global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid_constant__ MerkleLevelParams p) {
+    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
+    if (gid >= (unsigned long long)p.n_trees * p.n_out) return;
+    const unsigned t = (unsigned)(gid / p.n_out), j = (unsigned)(gid % p.n_out);
+    if (p.odd_trees_only_if_nonempty && (t & 1u)) return;
+    const unsigned lo = j * FANOUT, hi = min(lo + FANOUT, p.n_in), cnt = hi - lo;
+    const uint4 *src = reinterpret_cast<const uint4 *>(p.in + (size_t)t * p.in_tree_stride + (size_t)lo * 32);
+    uint32_t H[8];
+    sha256_init(H);
+    const unsigned pairs = cnt >> 1;
+    uint32_t w[16];
+#pragma unroll 1
+    for (unsigned i = 0; i <= pairs; ++i) {
+        // block i holds children 2i, 2i+1; the last iteration holds the odd child (if any) and the padding
+        if (i < pairs) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint4 v = __ldg(src + 4 * i + q);
+                w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) w[q] = 0u;
+            if (cnt & 1u) {
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    const uint4 v = __ldg(src + 4 * i + q);
+                    w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
+                }
+                w[8] = 0x80000000u;
+            } else {
+                w[0] = 0x80000000u;
+            }
+            w[15] = cnt * 256u;  // message bits = cnt * 32 bytes * 8
+        }
+        sha256_compress(H, w);
+    }
+    store_digest(p.out + (size_t)t * p.out_tree_stride + (size_t)j * 32, H);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Leaves of a byte stream: leaf j of stream t = SHA-256(bytes [j*LEAF, min((j+1)*LEAF, n))). One thread per leaf.
+// Stream length is a multiple of 4 bytes here (int16 pairs are guaranteed by even subband widths: every band
+// row has w>>l >= 1 elements but the whole fragment length is a multiple of 4 unless a band is 1 element wide;
+// the generic byte tail below handles any length).
+// ------------------------------------------------------------------------------------------------------------
+struct StreamLeavesParams {
+    const uint8_t *data;     // stream t at data + t*stream_stride
+    size_t stream_stride;
+    unsigned long long n_bytes;  // per stream
+    unsigned n_leaves;           // per stream
+    unsigned n_streams;
+    uint8_t *out;                // leaf digests [stream][leaf][32] with out_stream_stride bytes between streams
+    size_t out_stream_stride;
+};
+
+__global__ void __launch_bounds__(HASH_THREADS) stream_leaves_kernel(const __grid_constant__ StreamLeavesParams p) {
+    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
+    if (gid >= (unsigned long long)p.n_streams * p.n_leaves) return;
+    const unsigned t = (unsigned)(gid / p.n_leaves), j = (unsigned)(gid % p.n_leaves);
+    const unsigned long long lo = (unsigned long long)j * DWT_LEAF_BYTES;
+    const unsigned len = (unsigned)min((unsigned long long)DWT_LEAF_BYTES, p.n_bytes - lo);
+    const uint8_t *src = p.data + (size_t)t * p.stream_stride + lo;
+    uint32_t H[8];
+    sha256_init(H);
+    const unsigned full = len >> 6, tail = len & 63u;
+    const unsigned nblocks = full + ((tail + 9 <= 64) ? 1u : 2u);
+    uint32_t w[16];
+#pragma unroll 1
+    for (unsigned i = 0; i < nblocks; ++i) {
+        if (i < full) {
+            const uint4 *s4 = reinterpret_cast<const uint4 *>(src + 64 * (size_t)i);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const uint4 v = __ldg(s4 + q);
+                w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
+            }
+        } else {
+            // tail + padding, byte by byte (only the last leaf of a stream ever has a tail)
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                uint32_t word = 0;
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const unsigned pos = 64u * i + 4u * q + b;  // byte position within the leaf
+                    uint32_t byte = 0;
+                    if (pos < len) byte = src[pos];
+                    else if (pos == len) byte = 0x80u;
+                    word = (word << 8) | byte;
+                }
+                w[q] = word;
+            }
+            if (i == nblocks - 1) { w[14] = 0u; w[15] = len * 8u; }
+        }
+        sha256_compress(H, w);
+    }
+    store_digest(p.out + (size_t)t * p.out_stream_stride + (size_t)j * 32, H);
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// AES-128-CTR over a byte stream, in place: one thread per 16-byte block (A6). n_bytes per stream.
+// ------------------------------------------------------------------------------------------------------------
+struct CtrParams {
+    uint8_t *data;
+    size_t stream_stride;
+    unsigned long long n_bytes;
+    unsigned n_streams;
+    const uint8_t *d_nonces;
+    uint32_t nonce_be[4];
+    uint32_t rk[44];
+};
+
+__global__ void __launch_bounds__(HASH_THREADS) aes_ctr_kernel(const __grid_constant__ CtrParams p) {
+    __shared__ uint32_t sT[AES_TABLE_WORDS];
+    load_aes_tables(sT);
+    const unsigned long long nblk = (p.n_bytes + 15) >> 4;
+    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
+    if (gid >= nblk * p.n_streams) return;
+    const unsigned t = (unsigned)(gid / nblk);
+    const unsigned long long i = gid % nblk;
+    uint32_t nonce[4];
+    if (p.d_nonces) {
+        const uint4 q = __ldg(reinterpret_cast<const uint4 *>(p.d_nonces) + t);
+        nonce[0] = bswap32(q.x); nonce[1] = bswap32(q.y); nonce[2] = bswap32(q.z); nonce[3] = bswap32(q.w);
+    } else {
+        nonce[0] = p.nonce_be[0]; nonce[1] = p.nonce_be[1]; nonce[2] = p.nonce_be[2]; nonce[3] = p.nonce_be[3];
+    }
+    uint32_t ks[4];
+    ctr_block(nonce, i, ks);
+    aes128_encrypt(sT, p.rk, ks);
+    uint8_t *dst = p.data + (size_t)t * p.stream_stride + 16 * i;
+    if (16 * i + 16 <= p.n_bytes) {
+        uint4 v = *reinterpret_cast<uint4 *>(dst);
+        v.x ^= ks[0]; v.y ^= ks[1]; v.z ^= ks[2]; v.w ^= ks[3];
+        *reinterpret_cast<uint4 *>(dst) = v;
+    } else {
+        const unsigned rem = (unsigned)(p.n_bytes - 16 * i);
+        for (unsigned b = 0; b < rem; ++b) dst[b] ^= (uint8_t)(ks[b >> 2] >> (8 * (b & 3)));
+    }
+}
+
+// verify: flags[n] = bit0 (private root mismatch) | bit1 (public root mismatch); one thread per image
+__global__ void compare_digests_kernel(const uint8_t *computed, const uint8_t *expected, uint32_t *flags, int n_images) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_images) return;
+    const uint32_t *a = reinterpret_cast<const uint32_t *>(computed) + 16 * n;
+    const uint32_t *b = reinterpret_cast<const uint32_t *>(expected) + 16 * n;
+    uint32_t d0 = 0, d1 = 0;
+    for (int i = 0; i < 8; ++i) { d0 |= a[i] ^ b[i]; d1 |= a[8 + i] ^ b[8 + i]; }
+    flags[n] = (d0 ? 1u : 0u) | (d1 ? 2u : 0u);
+}
+
+// root of an empty fragment = SHA-256(""), written to digests[64 n + 32 .. 64 n + 63]
+__global__ void write_empty_public_root_kernel(uint8_t *digests, int n_images) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_images) return;
+    uint32_t H[8], w[16];
+    sha256_init(H);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) w[i] = 0u;
+    w[0] = 0x80000000u;
+    sha256_compress(H, w);
+    store_digest(digests + 64 * (size_t)n + 32, H);
+}
+
+}  // namespace feds

@@ -1,0 +1,248 @@
+"""GPU parity tests for the DCT path, through the C ABI (paper_1512_02951_b200.binding), against the CPU oracle.
+
+Two-stage protocol:
+  (i)   GPU coefficients (private part decrypted with the known key) vs the oracle's DOUBLE coefficients: max abs <= 1e-3
+        (BASELINE.json north_star tolerance: FP32 against the double oracle, 8-bit inputs);
+  (ii)  the oracle's pack + AES-CTR + SHA-256/Merkle fed the GPU's own float32 coefficient bytes: private ciphertext, public
+        bytes and both digests bit-exact;
+  (iii) reconstructions bit-exact uint8: GPU(GPU), oracle(GPU fragments), GPU(oracle fragments).
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def b():
+    from paper_1512_02951_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def gpu_coefficients(orc, priv, pub, nb, k, key, nonce):
+    """float32 [nb][64] zigzag-ordered coefficients recovered from the GPU fragments."""
+    pt = np.frombuffer(orc.aes128_ctr_xor(key, nonce, priv.tobytes()), dtype="<f4").reshape(nb, k + 1)
+    pu = np.frombuffer(pub.tobytes(), dtype="<f4").reshape(nb, 63 - k)
+    return np.concatenate([pt, pu], axis=1)
+
+
+def check_fragment_parity(orc, b, img, k, seed, check_coefficients=True):
+    h, w, c = img.shape
+    key, nonce = synth.key_nonce(seed)
+    d_img = torch.from_numpy(img).cuda()
+    priv, pub, dg = b.fragment_dct(d_img, k, key, nonce)
+    torch.cuda.synchronize()
+    priv, pub, dg = priv.cpu().numpy(), pub.cpu().numpy(), dg.cpu().numpy().tobytes()
+    nb = c * (h // 8) * (w // 8)
+    assert priv.size == orc.dct_private_bytes(w, h, c, k) and pub.size == orc.dct_public_bytes(w, h, c, k)
+    coef32 = gpu_coefficients(orc, priv, pub, nb, k, key, nonce)
+    if check_coefficients:                                                  # stage (i)
+        ref = orc.dct_coefficients(img)
+        err = np.abs(coef32.astype(np.float64) - ref).max()
+        assert err <= TOL, err
+    p2, q2, d2 = orc.fragment_from_coef32(coef32, w, h, c, k, key, nonce)   # stage (ii)
+    assert (p2 == priv).all(), "private ciphertext differs"
+    assert (q2 == pub).all(), "public bytes differ"
+    assert d2[:32] == dg[:32], "private digest differs"
+    assert d2[32:] == dg[32:], "public digest differs"
+    return d_img, priv, pub, dg, key, nonce
+
+
+CASES = [
+    (8, 8, 1, 0), (8, 8, 1, 63), (16, 16, 4, 63), (64, 8, 1, 3), (72, 24, 1, 5), (1080, 16, 3, 3), (136, 40, 4, 9),
+    (512, 512, 1, 2),      # BASELINE config 1
+    (256, 264, 3, 5), (1032, 8, 1, 2), (520, 24, 3, 31), (64, 64, 1, 32), (128, 16, 3, 62), (40, 8, 3, 4), (2056, 8, 1, 1),
+]
+
+
+@pytest.mark.parametrize("w,h,c,k", CASES)
+def test_fragment_parity_and_round_trips(orc, b, w, h, c, k):
+    img = synth.image(w, h, c, seed=w + 3 * h + c + k, rectangles=2 if w >= 64 and h >= 16 else 0)
+    d_img, priv, pub, dg, key, nonce = check_fragment_parity(orc, b, img, k, seed=w * 7 + k)
+    d_priv, d_pub = torch.from_numpy(priv).cuda(), torch.from_numpy(pub).cuda()
+    if pub.size == 0:
+        d_pub = torch.zeros(16, dtype=torch.uint8, device="cuda")
+    d_dg = torch.frombuffer(bytearray(dg), dtype=torch.uint8).cuda()
+    # (iii) GPU defragment of GPU fragments, with verification
+    rec, flags = b.defragment_dct(d_priv, d_pub, w, h, c, k, key, nonce, expected=d_dg)
+    torch.cuda.synchronize()
+    assert int(flags.item()) == 0
+    assert torch.equal(rec, d_img)
+    # without verification
+    rec2, _ = b.defragment_dct(d_priv, d_pub, w, h, c, k, key, nonce)
+    assert torch.equal(rec2, d_img)
+    # oracle defragment of GPU fragments
+    orec, oflags = orc.defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=dg)
+    assert oflags == 0 and (orec == img).all()
+    # GPU defragment of ORACLE fragments (whose coefficient bytes come from the double DCT)
+    op, oq, odg = orc.fragment_dct(img, k, key, nonce)
+    d_op = torch.from_numpy(op).cuda()
+    d_oq = torch.from_numpy(oq).cuda() if oq.size else torch.zeros(16, dtype=torch.uint8, device="cuda")
+    d_odg = torch.frombuffer(bytearray(odg), dtype=torch.uint8).cuda()
+    rec3, flags3 = b.defragment_dct(d_op, d_oq, w, h, c, k, key, nonce, expected=d_odg)
+    torch.cuda.synchronize()
+    assert int(flags3.item()) == 0 and torch.equal(rec3, d_img)
+
+
+@pytest.mark.parametrize("kind", ["zeros", "ones", "checker", "random", "impulse"])
+@pytest.mark.parametrize("c", [1, 3, 4])
+def test_special_images(orc, b, kind, c):
+    img = synth.special(kind, 96, 32, c, seed=c)
+    d_img, priv, pub, dg, key, nonce = check_fragment_parity(orc, b, img, 5, seed=11)
+    rec, flags = b.defragment_dct(torch.from_numpy(priv).cuda(), torch.from_numpy(pub).cuda(), 96, 32, c, 5, key, nonce,
+                                  expected=torch.frombuffer(bytearray(dg), dtype=torch.uint8).cuda())
+    torch.cuda.synchronize()
+    assert int(flags.item()) == 0 and torch.equal(rec, d_img)   # T6: lossless
+
+
+def test_dc_bound_on_device(orc, b):
+    img = np.full((8, 64, 1), 255, dtype=np.uint8)
+    key, nonce = synth.key_nonce(1)
+    priv, pub, _ = b.fragment_dct(torch.from_numpy(img).cuda(), 0, key, nonce)
+    dc = np.frombuffer(orc.aes128_ctr_xor(key, nonce, priv.cpu().numpy().tobytes()), dtype="<f4")
+    assert np.abs(dc - 2040.0).max() < 1e-3
+    assert np.abs(np.frombuffer(pub.cpu().numpy().tobytes(), dtype="<f4")).max() < 1e-3
+
+
+def test_verify_flags_and_error_confinement(orc, b):
+    w, h, c, k = 128, 32, 1, 3
+    img = synth.image(w, h, c, seed=6)
+    key, nonce = synth.key_nonce(6)
+    d_img = torch.from_numpy(img).cuda()
+    priv, pub, dg = b.fragment_dct(d_img, k, key, nonce)
+    p2 = priv.clone(); p2[99] ^= 0x40          # top byte of block 6's DC
+    rec, flags = b.defragment_dct(p2, pub, w, h, c, k, key, nonce, expected=dg)
+    assert int(flags.item()) == 1
+    diff = (rec != d_img)[:, :, 0].cpu().numpy()
+    mask = np.zeros_like(diff); mask[0:8, 48:56] = True
+    assert diff[mask].any() and not diff[~mask].any()            # CTR: damage confined to one 8x8 block
+    q2 = pub.clone(); q2[-1] ^= 1
+    _, flags = b.defragment_dct(priv, q2, w, h, c, k, key, nonce, expected=dg)
+    assert int(flags.item()) == 2
+    _, flags = b.defragment_dct(p2, q2, w, h, c, k, key, nonce, expected=dg)
+    assert int(flags.item()) == 3
+    bad, _ = b.defragment_dct(priv, pub, w, h, c, k, bytes(16), nonce)
+    assert (bad != d_img).float().mean().item() > 0.5            # wrong key does not reconstruct
+
+
+def test_counter_carry_on_device(orc, b):
+    # nonce just below the 32-bit and 64-bit carry boundaries (A6)
+    img = synth.image(64, 32, 1, seed=8)
+    key, _ = synth.key_nonce(8)
+    for nonce in [bytes.fromhex("000000000000000000000000fffffffe"), bytes.fromhex("0000000000000000fffffffffffffffe"),
+                  bytes.fromhex("fffffffffffffffffffffffffffffffd")]:
+        priv, pub, dg = b.fragment_dct(torch.from_numpy(img).cuda(), 3, key, nonce)
+        coef = gpu_coefficients(orc, priv.cpu().numpy(), pub.cpu().numpy(), 32, 3, key, nonce)
+        p2, q2, d2 = orc.fragment_from_coef32(coef, 64, 32, 1, 3, key, nonce)
+        assert (p2 == priv.cpu().numpy()).all() and d2 == dg.cpu().numpy().tobytes()
+        assert np.abs(coef - orc.dct_coefficients(img)).max() <= TOL
+
+
+def test_batch_equals_singles(orc, b):
+    n, w, h, c, k = 5, 136, 24, 3, 3
+    key, nonce = synth.key_nonce(21)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=100 + i, rectangles=1) for i in range(n)])
+    d_imgs = torch.from_numpy(imgs).cuda()
+    batch = b.DctBatch(n, w, h, c, k)
+    d_nonces = torch.from_numpy(nonces).cuda()
+    batch.fragment(d_imgs, key, d_nonces)
+    torch.cuda.synchronize()
+    for i in range(n):
+        pv, pb, dg = b.fragment_dct(d_imgs[i].contiguous(), k, key, nonces[i].tobytes())
+        assert torch.equal(pv, batch.priv[i * batch.priv_bytes:(i + 1) * batch.priv_bytes])
+        assert torch.equal(pb, batch.pub[i * batch.pub_bytes:(i + 1) * batch.pub_bytes])
+        assert torch.equal(dg, batch.digests[64 * i:64 * i + 64])
+    out = torch.empty_like(d_imgs)
+    batch.defragment(out, key, d_nonces, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    batch.pub[batch.pub_bytes * 3 + 5] ^= 0x80
+    batch.defragment(out, key, d_nonces, expected=batch.digests)
+    assert batch.flags_out.cpu().tolist() == [0, 0, 0, 2, 0]
+    # no-digest flag: same fragment bytes, digests untouched
+    batch2 = b.DctBatch(n, w, h, c, k)
+    batch2.digests.fill_(7)
+    batch2.fragment(d_imgs, key, d_nonces, flags=b.FLAG_NO_DIGEST)
+    torch.cuda.synchronize()
+    batch.pub[batch.pub_bytes * 3 + 5] ^= 0x80
+    assert torch.equal(batch2.priv, batch.priv) and torch.equal(batch2.pub, batch.pub) and bool((batch2.digests == 7).all())
+
+
+def test_host_staged_entry_point(orc, b):
+    n, w, h, c, k = 7, 64, 32, 3, 3
+    key, nonce = synth.key_nonce(31)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=200 + i) for i in range(n)])
+    h_imgs = torch.from_numpy(imgs).pin_memory()
+    h_non = torch.from_numpy(nonces).pin_memory()
+    pb_, qb_ = b.dct_private_bytes(w, h, c, k), b.dct_public_bytes(w, h, c, k)
+    h_priv = torch.empty(n * pb_, dtype=torch.uint8).pin_memory()
+    h_pub = torch.empty(n * qb_, dtype=torch.uint8).pin_memory()
+    h_dg = torch.empty(n * 64, dtype=torch.uint8).pin_memory()
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    scratch = torch.empty(b.host_scratch_bytes(2, 3, w, h, c, k), dtype=torch.uint8, device="cuda")
+    b.fragment_dct_host(h_imgs, w, h, c, k, key, h_non, h_priv, h_pub, h_dg, 2, scratch, streams)
+    for s in streams:
+        s.synchronize()
+    for i in range(n):
+        pv, pu, dg = b.fragment_dct(torch.from_numpy(imgs[i]).cuda(), k, key, nonces[i].tobytes())
+        assert (pv.cpu() == h_priv[i * pb_:(i + 1) * pb_]).all() and (pu.cpu() == h_pub[i * qb_:(i + 1) * qb_]).all()
+        assert (dg.cpu() == h_dg[64 * i:64 * i + 64]).all()
+
+
+# ---------------------------------------------------------------- full BASELINE sizes, in the configuration bench.py times
+def test_config2_full_size(orc, b):
+    """4096x4096 RGB, k=5: whole-image stage (ii) + round trip; coefficients on sampled crops (the double DCT is slow)."""
+    w = h = 4096; c = 3; k = 5
+    img = synth.image(w, h, c, seed=2)
+    d_img, priv, pub, dg, key, nonce = check_fragment_parity(orc, b, img, k, seed=2, check_coefficients=False)
+    nb = c * (h // 8) * (w // 8)
+    coef = gpu_coefficients(orc, priv, pub, nb, k, key, nonce).reshape(c, h // 8, w // 8, 64)
+    rng = np.random.default_rng(0)
+    for _ in range(6):
+        by, bx = int(rng.integers(0, h // 8 - 8)), int(rng.integers(0, w // 8 - 8))
+        crop = np.ascontiguousarray(img[8 * by:8 * by + 64, 8 * bx:8 * bx + 64, :])
+        ref = orc.dct_coefficients(crop).reshape(c, 8, 8, 64)
+        assert np.abs(coef[:, by:by + 8, bx:bx + 8, :] - ref).max() <= TOL
+    rec, flags = b.defragment_dct(torch.from_numpy(priv).cuda(), torch.from_numpy(pub).cuda(), w, h, c, k, key, nonce,
+                                  expected=torch.frombuffer(bytearray(dg), dtype=torch.uint8).cuda())
+    torch.cuda.synchronize()
+    assert int(flags.item()) == 0 and torch.equal(rec, d_img)
+
+
+def test_config3_batch_full_size(orc, b):
+    """256 x 1920x1080 RGB, k=3, batched as bench.py launches it; sampled images checked in full by the oracle."""
+    n, w, h, c, k = 256, 1920, 1080, 3, 3
+    key, nonce = synth.key_nonce(3)
+    nonces = synth.batch_nonces(nonce, n)
+    d_imgs = synth.image_batch_torch(n, w, h, c, seed=3000, device="cuda", rectangles=16)
+    d_nonces = torch.from_numpy(nonces).cuda()
+    batch = b.DctBatch(n, w, h, c, k)
+    batch.fragment(d_imgs, key, d_nonces)
+    torch.cuda.synchronize()
+    nb = c * (h // 8) * (w // 8)
+    for i in [0, 1, 100, 255]:
+        img = d_imgs[i].cpu().numpy()
+        priv = batch.priv[i * batch.priv_bytes:(i + 1) * batch.priv_bytes].cpu().numpy()
+        pub = batch.pub[i * batch.pub_bytes:(i + 1) * batch.pub_bytes].cpu().numpy()
+        dg = batch.digests[64 * i:64 * i + 64].cpu().numpy().tobytes()
+        nz = nonces[i].tobytes()
+        coef = gpu_coefficients(orc, priv, pub, nb, k, key, nz)
+        p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nz)
+        assert (p2 == priv).all() and (q2 == pub).all() and d2 == dg
+        crop = np.ascontiguousarray(img[512:576, 960:1024, :])
+        ref = orc.dct_coefficients(crop).reshape(c, 8, 8, 64)
+        assert np.abs(coef.reshape(c, h // 8, w // 8, 64)[:, 64:72, 120:128, :] - ref).max() <= TOL
+    out = torch.empty_like(d_imgs)
+    batch.defragment(out, key, d_nonces, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    # every image's digests are distinct (independent CTR messages, A20)
+    dgs = batch.digests.cpu().numpy().reshape(n, 64)
+    assert len({bytes(r[:32]) for r in dgs}) == n

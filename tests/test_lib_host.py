@@ -1,0 +1,125 @@
+"""CPU-only checks of libfeds.so: it loads, exports every symbol include/feds.h declares, answers the size queries,
+rejects bad arguments before touching the device, and its __host__ __device__ arithmetic building blocks (the very
+functions the kernels call) agree with outside libraries. No GPU compute is launched here."""
+import ctypes as C
+import hashlib
+import os
+import re
+
+import numpy as np
+import pytest
+import scipy.fft
+from cryptography.hazmat.primitives.ciphers import Cipher, algorithms, modes
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def b():
+    from paper_1512_02951_b200 import build
+    build.build()
+    from paper_1512_02951_b200 import binding
+    return binding
+
+
+def test_exports_every_declared_symbol(b):
+    header = open(os.path.join(ROOT, "include", "feds.h")).read()
+    declared = set(re.findall(r"\b(feds_[a-z0-9_]+)\s*\(", header))
+    declared -= {"feds_stream_t"}
+    assert declared == set(b.SYMBOLS), declared ^ set(b.SYMBOLS)
+    for name in declared:
+        assert hasattr(b.lib, name), name
+
+
+def test_format_constants_match_design(b):
+    assert b.merkle_params() == (8, 16, 2048)  # DESIGN.md 2.1 / 2.2
+
+
+def test_size_queries(b):
+    # SURVEY.md 8(a) sizes at the BASELINE configs
+    assert b.dct_private_bytes(512, 512, 1, 2) == 49152 and b.dct_public_bytes(512, 512, 1, 2) == 999424
+    assert b.dct_private_bytes(4096, 4096, 3, 5) == 18874368 and b.dct_public_bytes(4096, 4096, 3, 5) == 182452224
+    assert b.dct_private_bytes(1920, 1080, 3, 3) == 1555200 and b.dct_public_bytes(1920, 1080, 3, 3) == 23328000
+    assert b.dwt_private_bytes(8192, 8192, 1, 3) == 2097152 and b.dwt_public_bytes(8192, 8192, 1, 3) == 132120576
+    assert b.dct_public_bytes(16, 16, 1, 63) == 0
+    for bad in [(12, 16, 1, 3), (16, 16, 2, 3), (16, 16, 1, 64), (0, 16, 1, 3)]:
+        assert b.dct_private_bytes(*bad) == 0
+    assert b.dwt_private_bytes(16, 24, 1, 4) == 0 and b.dwt_private_bytes(16, 16, 1, 7) == 0
+    assert b.workspace_bytes(512, 512, 1, 2) > 0 and b.workspace_bytes(512, 512, 1, 2) % 256 == 0
+    assert b.workspace_bytes(8192, 8192, 1, 3, True) >= 2 * (4096 * 4096 + 2048 * 2048 + 1024 * 1024)
+
+
+def test_argument_errors_are_reported_before_any_launch(b):
+    key = bytes(16)
+    ok_ptr = C.c_void_p(0x1000)  # never dereferenced: every call below must fail in validation
+    f = b.lib.feds_fragment_dct
+    assert f(None, 16, 16, 1, 3, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 1      # null pointer
+    assert f(ok_ptr, 12, 16, 1, 3, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 2    # bad dims
+    assert f(ok_ptr, 16, 16, 2, 3, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 3    # bad channels
+    assert f(ok_ptr, 16, 16, 1, 64, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 3   # bad k
+    assert f(ok_ptr, 64, 64, 1, 3, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 8, None) == 4          # workspace too small
+    assert f(C.c_void_p(0x1001), 16, 16, 1, 3, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 6  # misaligned
+    g = b.lib.feds_fragment_dwt
+    assert g(ok_ptr, 16, 24, 1, 4, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 2
+    assert g(ok_ptr, 16, 16, 1, 0, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 3
+    assert g(ok_ptr, 64, 64, 1, 2, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 8, None) == 4
+    assert b.lib.feds_status_string(2) == b"bad dimensions"
+
+
+def test_binding_has_no_cpu_fallback():
+    src = open(os.path.join(ROOT, "paper_1512_02951_b200", "binding.py")).read()
+    assert "oracle" not in src.replace("no CPU fallback", "")
+    for f in os.listdir(os.path.join(ROOT, "paper_1512_02951_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_1512_02951_b200", "csrc", f)).read().replace("oracle/", "")
+
+
+# ---------------------------------------------------------------- device arithmetic, run on the host
+@pytest.mark.parametrize("n", [0, 1, 3, 55, 56, 63, 64, 65, 119, 120, 128, 1000, 2048])
+def test_device_sha256_compress(b, n):
+    msg = np.random.default_rng(n).integers(0, 256, n, dtype=np.uint8).tobytes()
+    out = (C.c_uint8 * 32)()
+    b.lib.feds_debug_sha256_host(msg, n, out)
+    assert bytes(out) == hashlib.sha256(msg).digest()
+
+
+def test_device_aes_ttables(b, kat):
+    out = (C.c_uint8 * 16)()
+    b.lib.feds_debug_aes128_host(bytes.fromhex(kat["fips197_B_key"]), bytes.fromhex(kat["fips197_B_in"]), out)
+    assert bytes(out).hex() == kat["fips197_B_out"]
+    b.lib.feds_debug_aes128_host(bytes.fromhex(kat["fips197_C1_key"]), bytes.fromhex(kat["fips197_C1_in"]), out)
+    assert bytes(out).hex() == kat["fips197_C1_out"]
+    rng = np.random.default_rng(1)
+    for _ in range(200):
+        key = rng.integers(0, 256, 16, dtype=np.uint8).tobytes()
+        blk = rng.integers(0, 256, 16, dtype=np.uint8).tobytes()
+        e = Cipher(algorithms.AES(key), modes.ECB()).encryptor()
+        b.lib.feds_debug_aes128_host(key, blk, out)
+        assert bytes(out) == e.update(blk) + e.finalize()
+
+
+def test_device_dct_factorisation(b):
+    rng = np.random.default_rng(2)
+    worst = 0.0
+    blocks = [rng.integers(0, 256, (8, 8)) for _ in range(300)]
+    blocks += [np.full((8, 8), 255), np.zeros((8, 8)), (np.indices((8, 8)).sum(0) % 2) * 255, rng.integers(0, 2, (8, 8)) * 255]
+    for x in blocks:
+        xin = np.ascontiguousarray(x, dtype=np.float32)
+        out = np.empty(64, dtype=np.float32)
+        b.lib.feds_debug_dct8x8_host(xin.ctypes.data, out.ctypes.data, 0)
+        ref = scipy.fft.dctn(x.astype(np.float64), norm="ortho")
+        worst = max(worst, np.abs(out.reshape(8, 8) - ref).max())
+        back = np.empty(64, dtype=np.float32)
+        b.lib.feds_debug_dct8x8_host(out.ctypes.data, back.ctypes.data, 1)
+        assert (np.rint(back.reshape(8, 8)) == x).all()       # exact uint8 round trip
+    assert worst < 1e-3, worst                                # BASELINE tolerance (host float32 ~ device float32 up to FMA contraction)
+
+
+def test_device_zigzag_table(b, paper_pins):
+    out = (C.c_int * 64)()
+    b.lib.feds_debug_zigzag_host(out)
+    zz = [(v // 8, v % 8) for v in out]
+    want = [tuple(int(t) for t in p.split(",")) for p in paper_pins["zigzag_first6"].split()]
+    assert zz[:6] == want
+    assert sorted(out) == list(range(64))
+    for a, c in zip(zz, zz[1:]):
+        assert max(abs(a[0] - c[0]), abs(a[1] - c[1])) == 1
