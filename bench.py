@@ -1,0 +1,428 @@
+#!/usr/bin/env python
+"""bench.py — the headline benchmark of feds-b200 (contract: see DESIGN.md section 8).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg1|cfg2|cfg3|cfg4]
+
+One "step" = one pass of the whole hot path over one batch of seeded synthetic images:
+  DCT workloads : feds_fragment_dct_batch (DCT + select + AES-CTR + SHA-256 Merkle) followed by
+                  feds_defragment_dct_batch with digest verification (decrypt + merge + IDCT + round).
+  DWT workload  : feds_fragment_dwt followed by feds_defragment_dwt with verification.
+`value` = MB (10^6 B) of input image that went through the step per second, whole job over all ranks, inputs already
+resident in HBM. `e2e` = the same through the host-buffer C-ABI calls, host<->device copies inside the timed region.
+The default workload is BASELINE.json configs[2] (256 x 1920x1080 RGB, k=3), the one north_star quotes the target on.
+With N > 1 (torchrun) every rank runs its own batch (weak scaling, no data-path collective).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload, on rank 0 only.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "image MB/s fragmented (DCT+select+AES+SHA) on 1 B200; % HBM roofline"
+UNIT = "MB/s"
+
+WORKLOADS = {
+    # name: (kind, n_images, w, h, c, k_or_levels, rectangles, description)
+    "cfg1": ("dct", 1, 512, 512, 1, 2, 0, "BASELINE configs[0]: 512x512 gray, k=2 (latency case)"),
+    "cfg2": ("dct", 1, 4096, 4096, 3, 5, 0, "BASELINE configs[1]: 4096x4096 RGB, k=5"),
+    "cfg3": ("dct", 256, 1920, 1080, 3, 3, 16, "BASELINE configs[2]: batch of 256 RGB 1920x1080, k=3"),
+    "cfg4": ("dwt", 1, 8192, 8192, 1, 3, 0, "BASELINE configs[3]: 8192x8192 gray, 3-level 5/3 DWT"),
+}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows, self.proc, self.idx = [], None, gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) < 9:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------------ reference / cpu baseline
+def oracle_sample_jobs(kind, w, h, c, kl, n_jobs, seed):
+    """A bounded sample of the workload for the CPU oracle: horizontal strips of the workload's images, each an image in
+    its own right for the unchanged oracle entry points (DCT: 120-row strips; DWT: 256-row strips)."""
+    import synth
+    rows = 120 if kind == "dct" else 256
+    rows = min(rows, h)
+    jobs = []
+    for j in range(n_jobs):
+        img = synth.image(w, rows, c, seed=seed + j, rectangles=0)
+        jobs.append(img)
+    return jobs
+
+
+def run_oracle_jobs(kind, jobs, kl, threads):
+    """fragment + verified defragment of every job with the oracle as it stands; returns (seconds, bytes processed)."""
+    from concurrent.futures import ThreadPoolExecutor
+    import oracle
+    import synth
+    key, nonce = synth.key_nonce(7)
+
+    def one(img):
+        h, w, c = img.shape
+        if kind == "dct":
+            p, q, d = oracle.fragment_dct(img, kl, key, nonce)
+            rec, fl = oracle.defragment_dct(p, q, w, h, c, kl, key, nonce, expected=d)
+        else:
+            p, q, d = oracle.fragment_dwt(img, kl, key, nonce)
+            rec, fl = oracle.defragment_dwt(p, q, w, h, c, kl, key, nonce, expected=d)
+        assert fl == 0 and (rec == img).all()
+        return img.size
+
+    oracle.lib()
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=threads) as ex:   # ctypes releases the GIL during the C calls
+        total = sum(ex.map(one, jobs))
+    return time.perf_counter() - t0, total
+
+
+def reference_arm(args, kind, n, w, h, c, kl, desc):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    threads = min(os.cpu_count() or 1, 16)
+    rows = min(120 if kind == "dct" else 256, h)
+    jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
+    times = []
+    for it in range(args.warmup + args.steps):
+        dt, nbytes = run_oracle_jobs(kind, jobs, kl, threads)
+        if it >= args.warmup:
+            times.append(dt)
+    total_t = sum(times)
+    value = nbytes * len(times) / total_t / 1e6
+    sample = "%d strips of %dx%dx%d per step (one per thread), oracle fragment + verified defragment" % (len(jobs), w, rows, c)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total_t / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": desc, "step": "fragment + verified defragment", "note": "CPU oracle on a bounded sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------------------ our arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--images", type=int, default=0, help="override the number of images in the batch (DCT workloads)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    kind, n, w, h, c, kl, rects, desc = WORKLOADS[args.workload]
+    if args.images > 0 and kind == "dct":
+        n = args.images
+    if args.impl == "reference":
+        return reference_arm(args, kind, n, w, h, c, kl, desc)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import synth
+    from paper_1512_02951_b200 import binding as B   # raises if libfeds.so is missing: there is no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    hbm_peak, sm_max_mhz, peak_src = peaks()
+
+    key, nonce = synth.key_nonce(3)
+    img_bytes = w * h * c
+    step_image_bytes = n * img_bytes
+    launches = {"n": 0}
+    prof_frag, prof_defrag = [], []
+
+    if kind == "dct":
+        nonces = synth.batch_nonces(nonce, n)
+        d_nonces = torch.from_numpy(nonces).to(dev)
+        d_imgs = synth.image_batch_torch(n, w, h, c, seed=3000 + 1000 * rank, device=dev, rectangles=rects)
+        d_out = torch.empty_like(d_imgs)
+        batch = B.DctBatch(n, w, h, c, kl, device=dev)
+        nl = c * (h // 8) * ((w // 8 + 7) // 8)
+        tree_launches = 0
+        m = nl
+        while m > 1:
+            m = (m + 15) // 16
+            tree_launches += 1
+        per_step_launches = (1 + tree_launches) + (1 + tree_launches + 1)
+
+        def step(record=False):
+            if record:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                B.profile_events(e0, e1)
+                prof_frag.append((e0, e1))
+            batch.fragment(d_imgs, key, d_nonces)
+            if record:
+                e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                B.profile_events(e2, e3)
+                prof_defrag.append((e2, e3))
+            batch.defragment(d_out, key, d_nonces, expected=batch.digests)
+            if record:
+                B.profile_events(None, None)
+            launches["n"] += per_step_launches
+    else:
+        d_img = synth.image_batch_torch(1, w, h, c, seed=4000 + rank, device=dev)[0].contiguous()
+        ws = torch.empty(B.workspace_bytes(w, h, c, kl, True), dtype=torch.uint8, device=dev)
+        state = {}
+
+        def tl(nbytes):
+            m, t = (nbytes + 2047) // 2048, 0
+            while m > 1:
+                m = (m + 15) // 16
+                t += 1
+            return t
+        per_dig = 2 + tl(B.dwt_private_bytes(w, h, c, kl)) + tl(B.dwt_public_bytes(w, h, c, kl))
+        per_step_launches = (kl + 1 + per_dig) + (per_dig + 1 + 1 + kl)
+
+        def step(record=False):
+            pv, pb, dg = B.fragment_dwt(d_img, kl, key, nonce, workspace=ws)
+            rec, fl = B.defragment_dwt(pv, pb, w, h, c, kl, key, nonce, expected=dg, workspace=ws)
+            state["rec"], state["fl"] = rec, fl
+            launches["n"] += per_step_launches
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # correctness of what is being timed: round trip exact, no verify flag raised
+    if kind == "dct":
+        assert torch.equal(d_out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    else:
+        assert torch.equal(state["rec"], d_img) and int(state["fl"].item()) == 0
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches["n"] = 0
+    barrier()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        step(record=True)
+    t1.record()
+    barrier()
+    clocks = sampler.stop()
+    elapsed_ms = t0.elapsed_time(t1)
+    if world > 1:
+        t = torch.tensor([elapsed_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(t.item())
+    ms_per_step = elapsed_ms / args.steps
+    value = world * step_image_bytes / (ms_per_step * 1e-3) / 1e6
+    gpu_launches = launches["n"]
+
+    # ---------------------------------------------------------------- roofline of the dominant kernel (live, CUDA events)
+    roofline, stages = None, {}
+    if kind == "dct":
+        P, Q = kl + 1, 63 - kl
+        frag_ms = statistics.mean(a.elapsed_time(b_) for a, b_ in prof_frag)
+        defrag_ms = statistics.mean(a.elapsed_time(b_) for a, b_ in prof_defrag)
+        # algorithmic HBM bytes per launch: read 1 B + write 4 B per pixel-channel + 64 B leaf digests per leaf
+        alg_bytes = n * (img_bytes * 5 + nl * 64)
+        # algorithmic ALU-pipe work: SHA-256 compressions x 1400 lane-ops + AES blocks x 500
+        nblk_leaf = 8
+        comp_per_leaf = (nblk_leaf * Q * 4 + 9 + 63) // 64 + (nblk_leaf * P * 4 + 9 + 63) // 64
+        leaves_full = c * (h // 8) * ((w // 8) // 8)
+        alu_ops = n * (leaves_full * comp_per_leaf * 1400.0 + (img_bytes // 64) * P * 4 / 16 * 500.0)
+        alu_peak = 148 * 64 * sm_max_mhz * 1e6 / 1e12  # Tlane-op/s: 148 SMs x 4 SMSP x 16 ALU-pipe lanes/clk (B300_MICROARCH rt_SMSP = 2)
+        achieved = alu_ops / (frag_ms * 1e-3) / 1e12
+        roofline = {"kernel": "fragment_dct_kernel<3,true>", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                    "unit": "Tlane-op/s (32-bit ALU-pipe ops: SHF/LOP3/IADD3/PRMT)", "frac": achieved / alu_peak,
+                    "peak_source": "derived: 148 SM x 64 ALU-pipe lanes/clk x %.0f MHz (DESIGN.md section 7)" % sm_max_mhz,
+                    "traffic": None, "ms_per_launch": frag_ms,
+                    "hbm_view": {"achieved": alg_bytes / (frag_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                 "frac": alg_bytes / (frag_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
+                                 "algorithmic_bytes_per_launch": alg_bytes}}
+        stages["fragment_kernel_MBps"] = step_image_bytes / (frag_ms * 1e-3) / 1e6
+        stages["defragment_verify_kernel_MBps"] = step_image_bytes / (defrag_ms * 1e-3) / 1e6
+        # the HBM-bound core: the same kernels with digests disabled (FEDS_FLAG_NO_DIGEST), timed alone after the main region
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        for i in range(3):
+            batch.fragment(d_imgs, key, d_nonces, flags=B.FLAG_NO_DIGEST)
+            batch.defragment(d_out, key, d_nonces, flags=B.FLAG_NO_DIGEST)
+        torch.cuda.synchronize()
+        reps = 5
+        ev[0].record()
+        for i in range(reps):
+            batch.fragment(d_imgs, key, d_nonces, flags=B.FLAG_NO_DIGEST)
+        ev[1].record()
+        for i in range(reps):
+            batch.defragment(d_out, key, d_nonces, flags=B.FLAG_NO_DIGEST)
+        ev[2].record()
+        torch.cuda.synchronize()
+        f_ms, d_ms = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        core_bytes = n * img_bytes * 5
+        stages["nodigest"] = {"fragment_MBps": step_image_bytes / (f_ms * 1e-3) / 1e6, "defragment_MBps": step_image_bytes / (d_ms * 1e-3) / 1e6,
+                              "fragment_hbm_GBps": core_bytes / (f_ms * 1e-3) / 1e9, "fragment_hbm_frac": core_bytes / (f_ms * 1e-3) / 1e9 / hbm_peak,
+                              "defragment_hbm_GBps": core_bytes / (d_ms * 1e-3) / 1e9, "defragment_hbm_frac": core_bytes / (d_ms * 1e-3) / 1e9 / hbm_peak}
+
+    # ---------------------------------------------------------------- end to end through the host-buffer C ABI
+    e2e = None
+    if kind == "dct" and not args.no_e2e:
+        ipc, ns = min(8, n), 4
+        streams = [torch.cuda.Stream(device=dev) for _ in range(ns)]
+        h_imgs = torch.empty(n * img_bytes, dtype=torch.uint8).pin_memory()
+        h_imgs.copy_(d_imgs.view(-1).cpu())
+        h_non = torch.from_numpy(nonces).pin_memory()
+        h_priv = torch.empty(n * batch.priv_bytes, dtype=torch.uint8).pin_memory()
+        h_pub = torch.empty(n * batch.pub_bytes, dtype=torch.uint8).pin_memory()
+        h_dg = torch.empty(n * 64, dtype=torch.uint8).pin_memory()
+        h_out = torch.empty(n * img_bytes, dtype=torch.uint8).pin_memory()
+        h_fl = torch.zeros(n, dtype=torch.int32).pin_memory()
+        scratch = torch.empty(max(B.host_scratch_bytes(ipc, ns, w, h, c, kl), B.defrag_host_scratch_bytes(ipc, ns, w, h, c, kl)),
+                              dtype=torch.uint8, device=dev)
+
+        def e2e_step():
+            B.fragment_dct_host(h_imgs, w, h, c, kl, key, h_non, h_priv, h_pub, h_dg, ipc, scratch, streams)
+            B.defragment_dct_host(h_priv, h_pub, n, w, h, c, kl, key, h_non, h_dg, h_out, h_fl, ipc, scratch, streams)
+
+        e2e_step()
+        torch.cuda.synchronize()
+        assert torch.equal(h_out, h_imgs) and int(h_fl.abs().sum().item()) == 0
+        barrier()
+        reps = max(2, min(args.steps, 3))
+        cur = torch.cuda.current_stream()
+        es, ee = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        es.record(cur)
+        for s_ in streams:
+            s_.wait_event(es)
+        for _ in range(reps):
+            e2e_step()
+        for s_ in streams:
+            cur.wait_event(s_.record_event())
+        ee.record(cur)
+        torch.cuda.synchronize()
+        dt = es.elapsed_time(ee) * 1e-3 / reps   # device time from the first H2D to the last D2H, all streams joined
+        if world > 1:
+            t = torch.tensor([dt], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        frag_bytes = n * (batch.priv_bytes + batch.pub_bytes)
+        e2e = {"value": world * step_image_bytes / dt / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": n * img_bytes + 2 * n * 16 + frag_bytes + n * 64,
+               "d2h_bytes_per_step": frag_bytes + n * 64 + n * img_bytes + n * 4,
+               "ms_per_step": dt * 1e3, "streams": ns, "images_per_chunk": ipc, "host_memory": "pinned"}
+        gpu_launches += 0  # e2e launches are outside the timed region counted above
+    elif kind == "dwt" and not args.no_e2e:
+        # the DWT entry points take device pointers; e2e = pinned H2D of the image + D2H of fragments, digests and the image
+        h_img = d_img.cpu().pin_memory()
+        h_out = torch.empty_like(h_img).pin_memory()
+        pvb, pbb = B.dwt_private_bytes(w, h, c, kl), B.dwt_public_bytes(w, h, c, kl)
+        h_pv = torch.empty(pvb, dtype=torch.uint8).pin_memory()
+        h_pb = torch.empty(pbb, dtype=torch.uint8).pin_memory()
+        h_dg = torch.empty(64, dtype=torch.uint8).pin_memory()
+        d_in = torch.empty_like(d_img)
+
+        def e2e_step():
+            d_in.copy_(h_img, non_blocking=True)
+            pv, pb, dg = B.fragment_dwt(d_in, kl, key, nonce, workspace=ws)
+            h_pv.copy_(pv, non_blocking=True); h_pb.copy_(pb, non_blocking=True); h_dg.copy_(dg, non_blocking=True)
+            rec, fl = B.defragment_dwt(pv, pb, w, h, c, kl, key, nonce, expected=dg, workspace=ws)
+            h_out.copy_(rec, non_blocking=True)
+            return fl
+
+        e2e_step(); torch.cuda.synchronize()
+        tw = time.perf_counter()
+        reps = 3
+        for _ in range(reps):
+            e2e_step()
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - tw) / reps
+        assert torch.equal(h_out, h_img)
+        e2e = {"value": world * step_image_bytes / dt / 1e6, "unit": UNIT, "h2d_bytes_per_step": img_bytes,
+               "d2h_bytes_per_step": pvb + pbb + 64 + img_bytes, "ms_per_step": dt * 1e3, "host_memory": "pinned"}
+
+    # ---------------------------------------------------------------- CPU oracle baseline (rank 0, N = 1 only)
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        threads = min(os.cpu_count() or 1, 16)
+        rows = min(120 if kind == "dct" else 256, h)
+        jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
+        dt, nbytes = run_oracle_jobs(kind, jobs, kl, threads)
+        cpu_baseline = {"value": nbytes / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": "%d strips of %dx%dx%d (one per thread), fragment + verified defragment, %.1f s wall" % (len(jobs), w, rows, c, dt)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if kind == "dct" else "int16", "data": "synthetic",
+            "config": {"workload": desc, "step": "fragment + verified defragment (all SURVEY 8(a) rows)", "images_per_rank": n,
+                       "width": w, "height": h, "channels": c, "k_or_levels": kl,
+                       "l2": "inputs+outputs per step (%.1f GB) exceed the 126 MB L2; no flush needed" % ((step_image_bytes * 10) / 1e9)
+                       if step_image_bytes * 10 > 4e8 else "working set fits L2: cached numbers, reported as latency",
+                       "parallelism": "replicas (batch split), no collective"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "stages": stages,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

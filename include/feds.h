@@ -138,6 +138,25 @@ feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w,
                                    size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags);
 
 /*
+ * Host-staged batch defragment: the mirror image (H2D fragments + nonces [+ expected digests] -> defragment -> D2H
+ * images [+ verify flags]). h_expected_digests may be NULL (no verification; h_verify_flags untouched).
+ * Uses the same chunk -> stream mapping as feds_fragment_dct_host, so the two may be enqueued back to back on the same
+ * streams without a synchronisation in between.
+ */
+size_t feds_defragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k);
+feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_public, int n_images, int w, int h, int c, int k,
+                                     const uint8_t key[16], const uint8_t *h_nonces, const uint8_t *h_expected_digests,
+                                     uint8_t *h_images_out, uint32_t *h_verify_flags, int images_per_chunk, void *d_scratch,
+                                     size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags);
+
+/*
+ * Profiling hook (not part of the data path; thread-local): while set, every DCT fragment/defragment call made on this
+ * thread records ev_start immediately before and ev_stop immediately after its fused tile kernel, on the call's stream.
+ * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.
+ */
+void feds_profile_events(void *ev_start, void *ev_stop);
+
+/*
  * Host-side arithmetic self-checks of the device building blocks (the same __host__ __device__ functions the
  * kernels call), usable without a GPU. Not part of the data path.
  *   feds_debug_sha256_host   : SHA-256 of a host buffer through the kernels' compression function.

@@ -9,7 +9,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfeds.so")
+LIB_PATH = os.environ.get("FEDS_LIB_PATH") or os.path.join(_HERE, "libfeds.so")
 
 FLAG_NONE = 0
 FLAG_NO_DIGEST = 1
@@ -25,6 +25,7 @@ SYMBOLS = [
     "feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
     "feds_fragment_dct_batch", "feds_defragment_dct_batch",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
+    "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
 ]
 
@@ -58,12 +59,17 @@ def _load():
     lib.feds_fragment_dct_host_scratch_bytes.restype = sz
     lib.feds_fragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_fragment_dct_host.argtypes = [vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
+    lib.feds_defragment_dct_host_scratch_bytes.restype = sz
+    lib.feds_defragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
+    lib.feds_defragment_dct_host.argtypes = [vp, vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
+    lib.feds_profile_events.argtypes = [vp, vp]
+    lib.feds_profile_events.restype = None
     lib.feds_debug_sha256_host.argtypes = [u8p, sz, vp]
     lib.feds_debug_aes128_host.argtypes = [u8p, u8p, vp]
     lib.feds_debug_dct8x8_host.argtypes = [vp, vp, i]
     lib.feds_debug_zigzag_host.argtypes = [vp]
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
-                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host"]:
+                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host"]:
         getattr(lib, name).restype = i
     return lib
 
@@ -209,3 +215,26 @@ def fragment_dct_host(h_images, w, h, c, k, key, h_nonces, h_priv, h_pub, h_dige
 
 def host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k):
     return lib.feds_fragment_dct_host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k)
+
+
+def defragment_dct_host(h_priv, h_pub, n, w, h, c, k, key, h_nonces, h_expected, h_images_out, h_flags, images_per_chunk, d_scratch,
+                        streams, flags=FLAG_NONE):
+    """feds_defragment_dct_host: pinned host tensors in/out, staged over `streams`."""
+    arr = (C.c_void_p * len(streams))(*[s.cuda_stream for s in streams])
+    _check(lib.feds_defragment_dct_host(_ptr(h_priv), _ptr(h_pub), n, w, h, c, k, bytes(key), _ptr(h_nonces), _ptr(h_expected),
+                                        _ptr(h_images_out), _ptr(h_flags), images_per_chunk, _ptr(d_scratch), d_scratch.numel(), arr,
+                                        len(streams), flags), "feds_defragment_dct_host")
+
+
+def defrag_host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k):
+    return lib.feds_defragment_dct_host_scratch_bytes(images_per_chunk, n_streams, w, h, c, k)
+
+
+def profile_events(ev_start=None, ev_stop=None):
+    """Thread-local hook: record the two torch.cuda.Event objects around the fused tile kernel of subsequent DCT calls."""
+    for ev in (ev_start, ev_stop):
+        if ev is not None and not ev.cuda_event:
+            ev.record()  # torch creates the cudaEvent_t lazily; the library re-records it around the kernel
+    a = C.c_void_p(ev_start.cuda_event) if ev_start is not None else None
+    b_ = C.c_void_p(ev_stop.cuda_event) if ev_stop is not None else None
+    lib.feds_profile_events(a, b_)

@@ -9,7 +9,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libfeds.so")
+LIB = os.environ.get("FEDS_LIB_PATH") or os.path.join(HERE, "libfeds.so")
 SOURCES = ["feds_api.cu"]
 HEADERS = ["feds_device.cuh", "feds_dct.cuh", "feds_hash.cuh", "feds_dwt.cuh", os.path.join("..", "..", "include", "feds.h")]
 
@@ -37,7 +37,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+    extra = os.environ.get("FEDS_NVCC_EXTRA", "").split()
+    cmd = [nvcc] + NVCC_FLAGS + extra + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     log = os.path.join(HERE, "build.log")
     with open(log, "w") as f:

@@ -16,6 +16,7 @@ using namespace feds;
 namespace {
 
 thread_local int t_last_cuda_error = 0;
+thread_local cudaEvent_t t_prof_start = nullptr, t_prof_stop = nullptr;
 constexpr AesTables h_aes = make_aes_tables();
 constexpr ZigzagTable h_zigzag = make_zigzag();
 
@@ -120,42 +121,47 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.nbr = h / 8; p.nbc = w / 8; p.nlr = (p.nbc + G_BLOCKS - 1) / G_BLOCKS;
     p.leaves_per_image = (unsigned)c * p.nbr * p.nlr;
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
-    p.slot_stride = dct_slot_words(k, digest);
+    p.slot_stride = dct_slot_words(k);
+    (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
     aes128_expand_key_host(key, p.rk, h_aes);
 }
 
-template <bool DIGEST>
-feds_status launch_fragment(const DctParams &p, int c, cudaStream_t stream) {
+template <template <int, int> class Launcher>
+feds_status dispatch_cv(const DctParams &p, int c, cudaStream_t stream) {
+    const int V = dct_vec_width(p.k);
+#define FEDS_V(CC)                                                                  \
+    (V == 4 ? Launcher<CC, 4>::go(p, stream) : V == 2 ? Launcher<CC, 2>::go(p, stream) : Launcher<CC, 1>::go(p, stream))
+    return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
+#undef FEDS_V
+}
+
+template <typename Kernel>
+feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream) {
     const size_t smem = (size_t)(AES_TABLE_WORDS + DCT_THREADS * p.slot_stride) * 4;
     const unsigned grid = (unsigned)((p.total_leaves + DCT_THREADS - 1) / DCT_THREADS);
-#define FEDS_GO(CC)                                                                         \
-    {                                                                                       \
-        feds_status s = set_smem(fragment_dct_kernel<CC, DIGEST>, smem);                    \
-        if (s != FEDS_OK) return s;                                                         \
-        fragment_dct_kernel<CC, DIGEST><<<grid, DCT_THREADS, smem, stream>>>(p);            \
-    }
-    if (c == 1) FEDS_GO(1) else if (c == 3) FEDS_GO(3) else FEDS_GO(4)
-#undef FEDS_GO
+    feds_status s = set_smem(kernel, smem);
+    if (s != FEDS_OK) return s;
+    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
+    kernel<<<grid, DCT_THREADS, smem, stream>>>(p);
+    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;
 }
 
+template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, true>, p, s); } };
+template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, false>, p, s); } };
+template <int C, int V> struct DefragVerify { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, true>, p, s); } };
+template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, false>, p, s); } };
+
+template <bool DIGEST>
+feds_status launch_fragment(const DctParams &p, int c, cudaStream_t stream) {
+    return DIGEST ? dispatch_cv<FragDigest>(p, c, stream) : dispatch_cv<FragPlain>(p, c, stream);
+}
 template <bool VERIFY>
 feds_status launch_defragment(const DctParams &p, int c, cudaStream_t stream) {
-    const size_t smem = (size_t)(AES_TABLE_WORDS + DCT_THREADS * p.slot_stride) * 4;
-    const unsigned grid = (unsigned)((p.total_leaves + DCT_THREADS - 1) / DCT_THREADS);
-#define FEDS_GO(CC)                                                                         \
-    {                                                                                       \
-        feds_status s = set_smem(defragment_dct_kernel<CC, VERIFY>, smem);                  \
-        if (s != FEDS_OK) return s;                                                         \
-        defragment_dct_kernel<CC, VERIFY><<<grid, DCT_THREADS, smem, stream>>>(p);          \
-    }
-    if (c == 1) FEDS_GO(1) else if (c == 3) FEDS_GO(3) else FEDS_GO(4)
-#undef FEDS_GO
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
+    return VERIFY ? dispatch_cv<DefragVerify>(p, c, stream) : dispatch_cv<DefragPlain>(p, c, stream);
 }
 
 feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
@@ -544,6 +550,57 @@ feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w,
         if (digest) FEDS_CUDA(cudaMemcpyAsync(h_digests + (size_t)i0 * 64, d_dg, (size_t)m * 64, cudaMemcpyDeviceToHost, s));
     }
     return FEDS_OK;
+}
+
+size_t feds_defragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k) {
+    if (images_per_chunk < 1 || n_streams < 1 || check_dct_args(1, w, h, c, k) != FEDS_OK) return 0;
+    return (host_slot_bytes(images_per_chunk, w, h, c, k) + round_up((size_t)images_per_chunk * 4, 256)) * (size_t)n_streams;
+}
+
+feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_public, int n_images, int w, int h, int c, int k,
+                                     const uint8_t key[16], const uint8_t *h_nonces, const uint8_t *h_expected_digests,
+                                     uint8_t *h_images_out, uint32_t *h_verify_flags, int images_per_chunk, void *d_scratch,
+                                     size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags) {
+    feds_status st = check_dct_args(n_images, w, h, c, k);
+    if (st != FEDS_OK) return st;
+    if (images_per_chunk < 1 || n_streams < 1 || (flags & ~FEDS_FLAG_NO_DIGEST)) return FEDS_ERR_BAD_PARAM;
+    const bool verify = h_expected_digests != nullptr && !(flags & FEDS_FLAG_NO_DIGEST);
+    const size_t img_b = (size_t)w * h * c, priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
+    if (!h_private || (!h_public && pub_b) || !key || !h_nonces || !h_images_out || (verify && !h_verify_flags) || !d_scratch || !streams)
+        return FEDS_ERR_NULL_POINTER;
+    if (misaligned(d_scratch)) return FEDS_ERR_MISALIGNED;
+    const int ipc = images_per_chunk;
+    const size_t slot = host_slot_bytes(ipc, w, h, c, k) + round_up((size_t)ipc * 4, 256);
+    if (scratch_bytes < slot * (size_t)n_streams) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    const size_t ws_b = feds_workspace_bytes(w, h, c, k, 0);
+    int chunk = 0;
+    for (int i0 = 0; i0 < n_images; i0 += ipc, ++chunk) {
+        const int m = (n_images - i0 < ipc) ? n_images - i0 : ipc;
+        cudaStream_t s = streams[chunk % n_streams];
+        uint8_t *base = static_cast<uint8_t *>(d_scratch) + slot * (size_t)(chunk % n_streams);
+        uint8_t *d_img = base;
+        uint8_t *d_non = d_img + round_up((size_t)ipc * img_b, 256);
+        uint8_t *d_pv = d_non + round_up((size_t)ipc * 16, 256);
+        uint8_t *d_pb = d_pv + round_up((size_t)ipc * priv_b, 256);
+        uint8_t *d_dg = d_pb + round_up((size_t)ipc * pub_b, 256);
+        uint8_t *d_ws = d_dg + round_up((size_t)ipc * 64, 256);
+        uint32_t *d_fl = reinterpret_cast<uint32_t *>(d_ws + round_up((size_t)ipc * ws_b, 256));
+        FEDS_CUDA(cudaMemcpyAsync(d_pv, h_private + (size_t)i0 * priv_b, (size_t)m * priv_b, cudaMemcpyHostToDevice, s));
+        if (pub_b) FEDS_CUDA(cudaMemcpyAsync(d_pb, h_public + (size_t)i0 * pub_b, (size_t)m * pub_b, cudaMemcpyHostToDevice, s));
+        FEDS_CUDA(cudaMemcpyAsync(d_non, h_nonces + (size_t)i0 * 16, (size_t)m * 16, cudaMemcpyHostToDevice, s));
+        if (verify) FEDS_CUDA(cudaMemcpyAsync(d_dg, h_expected_digests + (size_t)i0 * 64, (size_t)m * 64, cudaMemcpyHostToDevice, s));
+        st = defragment_dct_impl(d_pv, priv_b, d_pb, pub_b, m, w, h, c, k, key, d_non, nullptr, verify ? d_dg : nullptr, d_img, img_b, d_fl,
+                                 d_ws, (size_t)ipc * ws_b, flags, s);
+        if (st != FEDS_OK) return st;
+        FEDS_CUDA(cudaMemcpyAsync(h_images_out + (size_t)i0 * img_b, d_img, (size_t)m * img_b, cudaMemcpyDeviceToHost, s));
+        if (verify) FEDS_CUDA(cudaMemcpyAsync(h_verify_flags + i0, d_fl, (size_t)m * 4, cudaMemcpyDeviceToHost, s));
+    }
+    return FEDS_OK;
+}
+
+void feds_profile_events(void *ev_start, void *ev_stop) {
+    t_prof_start = static_cast<cudaEvent_t>(ev_start);
+    t_prof_stop = static_cast<cudaEvent_t>(ev_stop);
 }
 
 // ------------------------------------------------------------------------------------------------ host self-checks

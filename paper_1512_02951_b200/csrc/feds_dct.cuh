@@ -2,22 +2,29 @@
 //
 // One thread owns one Merkle leaf = up to G consecutive 8x8 blocks of one block row of one channel
 // (DESIGN.md 2.1). For each block it: loads the 8x8 pixels, runs the separable FP32 DCT in 64 registers,
-// splits the coefficients in zigzag order into its private / public words in a per-lane shared-memory slot,
-// AES-128-CTR-encrypts the private words (shared-memory T-tables, sequential keystream along the leaf),
-// lets the warp copy both runs out to HBM coalesced, and absorbs the stored bytes of both fragments into two
-// running SHA-256 states (one inlined compression site). Pixels are read once; coefficients are written once;
-// only 2 x 32 B of leaf digest per leaf go to the workspace.
+// splits the coefficients in zigzag order into its private / public words, AES-128-CTR-encrypts the private
+// words (shared-memory T-tables, sequential keystream along the leaf), writes both runs to HBM, and absorbs the
+// stored bytes of both fragments into two running SHA-256 states fed from a per-lane shared-memory slot (one
+// inlined compression site). Pixels are read once; coefficients are written once; only 2 x 32 B of leaf digest
+// per leaf go to the workspace.
+//
+// Template parameter V = words per vector access of a coefficient run, the largest of {4, 2, 1} dividing
+// P = k+1 (then it divides Q = 64-P too, and every run starts 4V-byte aligned):
+//   V = 4 / 2 : each lane moves its own runs with 128 / 64-bit accesses straight from / to registers; no warp
+//               cooperation, no barrier in the block loop.
+//   V = 1     : 4-byte runs would scatter 64 stores per block over 32 lines each, so the warp copies every
+//               lane's runs through the slots with coalesced 32-bit accesses instead.
 #pragma once
 #include "feds_device.cuh"
 
 namespace feds {
 
 __device__ const AesTables g_aes = make_aes_tables();
-__device__ const ZigzagTable g_zigzag_unused = make_zigzag();  // (kept for cuobjdump inspection; kernels use the constexpr)
 
-constexpr int DCT_THREADS = 128;
+constexpr int DCT_THREADS = 256;
+constexpr int DCT_CTAS_PER_SM = 2;
 constexpr int AES_TABLE_WORDS = 1024;
-constexpr int CARRY = 15;  // a SHA-256 block is 16 words: at most 15 words are carried between blocks
+constexpr int CA = 16;  // carry area: a SHA-256 block is 16 words, at most 15 (16 - V) words wait between blocks
 
 struct DctParams {
     const uint8_t *images;  // fragment: input images; defragment: unused
@@ -35,15 +42,44 @@ struct DctParams {
     int nbr, nbc, nlr;
     unsigned leaves_per_image;  // C * nbr * nlr
     unsigned long long total_leaves;
-    int slot_stride;  // words per lane slot (odd)
+    int slot_stride;  // words per lane slot
 };
 
-// slot layout (word offsets in a lane's slot): private region [0, 15+P), public region [15+P, 30+64) (+ slack so
-// that the 32 padding words of the final phase fit after the public carry area)
-__host__ __device__ inline int dct_slot_words(int k, bool digest) {
-    const int Q = 63 - k;
-    int wds = digest ? (2 * CARRY + 64 + (Q < 32 ? 32 - Q : 0)) : 64 + 2 * CARRY;
-    return wds | 1;
+// Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:
+//   [0, 16)        private carry        [16, 16+P)       private words of the current block, index z
+//   [16+P, 32+P)   public carry         [32+P, 96)       public words of the current block, index z (address 32 + z)
+// plus slack so that the <= 32 padding words of the final phase fit behind the public carry area.
+// The stride makes per-lane V-word accesses conflict-free: odd (V=1), 2 mod 4 (V=2), 4 mod 8 (V=4).
+__host__ __device__ inline int dct_vec_width(int k) { return ((k + 1) % 4 == 0) ? 4 : ((k + 1) % 2 == 0) ? 2 : 1; }
+__host__ __device__ inline int dct_slot_words(int k) {
+    const int Q = 63 - k, V = dct_vec_width(k);
+    int wds = 2 * CA + 64 + (Q < 32 ? 32 - Q : 0);
+    while (wds % (2 * V) != V) ++wds;
+    return wds;
+}
+
+template <int V> struct VecT;
+template <> struct VecT<1> { using type = uint32_t; };
+template <> struct VecT<2> { using type = uint2; };
+template <> struct VecT<4> { using type = uint4; };
+
+template <int V>
+__device__ __forceinline__ void vec_store(uint32_t *dst, const uint32_t (&x)[V]) {
+    if (V == 1) dst[0] = x[0];
+    else if (V == 2) *reinterpret_cast<uint2 *>(dst) = make_uint2(x[0], x[1]);
+    else *reinterpret_cast<uint4 *>(dst) = make_uint4(x[0], x[1 % V], x[2 % V], x[3 % V]);
+}
+template <int V>
+__device__ __forceinline__ void vec_load(const uint32_t *src, uint32_t (&x)[V]) {
+    if (V == 1) x[0] = src[0];
+    else if (V == 2) { const uint2 t = *reinterpret_cast<const uint2 *>(src); x[0] = t.x; x[1 % V] = t.y; }
+    else { const uint4 t = *reinterpret_cast<const uint4 *>(src); x[0] = t.x; x[1 % V] = t.y; x[2 % V] = t.z; x[3 % V] = t.w; }
+}
+template <int V>
+__device__ __forceinline__ void vec_load_global(const uint32_t *src, uint32_t (&x)[V]) {
+    if (V == 1) x[0] = __ldg(src);
+    else if (V == 2) { const uint2 t = __ldg(reinterpret_cast<const uint2 *>(src)); x[0] = t.x; x[1 % V] = t.y; }
+    else { const uint4 t = __ldg(reinterpret_cast<const uint4 *>(src)); x[0] = t.x; x[1 % V] = t.y; x[2 % V] = t.z; x[3 % V] = t.w; }
 }
 
 template <int C>
@@ -80,26 +116,80 @@ __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int 
     }
 }
 
+// Round to nearest even, clamp to [0,255] (A5) and store the 8x8 block of channel c.
+// C == 1: one 8-byte store per row. C == 3 / 4: the C lanes holding the channels of one pixel strip are adjacent
+// (channel-fastest leaf order); lane c == 0 gathers its partners' rows with shuffles, interleaves them with byte
+// permutes and stores whole 8*C-byte row segments. Strips whose C lanes straddle a warp fall back to byte stores.
 template <int C>
-__device__ __forceinline__ void store_block(uint8_t *__restrict__ img, int w, int y0, int x0, int c, const float (&v)[64]) {
+__device__ __forceinline__ void store_block(uint8_t *__restrict__ img, int w, int y0, int x0, int c, bool act, const float (&v)[64]) {
+    const int lane = threadIdx.x & 31;
+    bool complete = true;
+    if (C > 1) {
+        // all C lanes of my strip are in this warp, and all are active
+        const int l0 = lane - c;
+        complete = (l0 >= 0) && (l0 + C - 1 <= 31);
+        const unsigned actmask = __ballot_sync(0xffffffffu, act);
+        if (complete) complete = ((actmask >> l0) & ((1u << C) - 1u)) == ((1u << C) - 1u);
+    }
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         uint32_t px[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
-            int q = __float2int_rn(v[8 * r + i]);  // round to nearest even (A5)
+            int q = __float2int_rn(v[8 * r + i]);
             q = min(max(q, 0), 255);
             px[i] = (uint32_t)q;
         }
-        uint8_t *row = img + ((size_t)(y0 + r) * w + x0) * C;
+        const uint32_t lo = px[0] | (px[1] << 8) | (px[2] << 16) | (px[3] << 24);
+        const uint32_t hi = px[4] | (px[5] << 8) | (px[6] << 16) | (px[7] << 24);
+        uint8_t *row = img + ((size_t)(y0 + r) * w + x0) * C;  // start of the strip's 8*C-byte row segment
         if (C == 1) {
-            uint2 q;
-            q.x = px[0] | (px[1] << 8) | (px[2] << 16) | (px[3] << 24);
-            q.y = px[4] | (px[5] << 8) | (px[6] << 16) | (px[7] << 24);
-            *reinterpret_cast<uint2 *>(row) = q;
-        } else {
+            if (act) *reinterpret_cast<uint2 *>(row) = make_uint2(lo, hi);
+        } else if (C == 3) {
+            const uint32_t glo = __shfl_down_sync(0xffffffffu, lo, 1), ghi = __shfl_down_sync(0xffffffffu, hi, 1);
+            const uint32_t blo = __shfl_down_sync(0xffffffffu, lo, 2), bhi = __shfl_down_sync(0xffffffffu, hi, 2);
+            if (complete) {
+                if (c == 0) {
+                    // bytes: R = lo/hi, G = glo/ghi, B = blo/bhi; output RGB RGB ...
+                    const uint32_t rg0 = __byte_perm(lo, glo, 0x5140);   // R0 G0 R1 G1
+                    const uint32_t rg1 = __byte_perm(lo, glo, 0x7362);   // R2 G2 R3 G3
+                    const uint32_t rg2 = __byte_perm(hi, ghi, 0x5140);   // R4 G4 R5 G5
+                    const uint32_t rg3 = __byte_perm(hi, ghi, 0x7362);   // R6 G6 R7 G7
+                    const uint32_t w0 = __byte_perm(rg0, blo, 0x2410);   // R0 G0 B0 R1
+                    const uint32_t w1 = __byte_perm(__byte_perm(rg0, blo, 0x0053), rg1, 0x5410);  // G1 B1 R2 G2
+                    const uint32_t w2 = __byte_perm(rg1, blo, 0x7326);   // B2 R3 G3 B3
+                    const uint32_t w3 = __byte_perm(rg2, bhi, 0x2410);
+                    const uint32_t w4 = __byte_perm(__byte_perm(rg2, bhi, 0x0053), rg3, 0x5410);
+                    const uint32_t w5 = __byte_perm(rg3, bhi, 0x7326);
+                    uint2 *o = reinterpret_cast<uint2 *>(row);
+                    o[0] = make_uint2(w0, w1);
+                    o[1] = make_uint2(w2, w3);
+                    o[2] = make_uint2(w4, w5);
+                }
+            } else if (act) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) row[i * C + c] = (uint8_t)px[i];
+                for (int i = 0; i < 8; ++i) row[i * 3 + c] = (uint8_t)px[i];
+            }
+        } else {
+            const uint32_t glo = __shfl_down_sync(0xffffffffu, lo, 1), ghi = __shfl_down_sync(0xffffffffu, hi, 1);
+            const uint32_t blo = __shfl_down_sync(0xffffffffu, lo, 2), bhi = __shfl_down_sync(0xffffffffu, hi, 2);
+            const uint32_t alo = __shfl_down_sync(0xffffffffu, lo, 3), ahi = __shfl_down_sync(0xffffffffu, hi, 3);
+            if (complete) {
+                if (c == 0) {
+                    const uint32_t rg0 = __byte_perm(lo, glo, 0x5140), rg1 = __byte_perm(lo, glo, 0x7362);
+                    const uint32_t ba0 = __byte_perm(blo, alo, 0x5140), ba1 = __byte_perm(blo, alo, 0x7362);
+                    const uint32_t rg2 = __byte_perm(hi, ghi, 0x5140), rg3 = __byte_perm(hi, ghi, 0x7362);
+                    const uint32_t ba2 = __byte_perm(bhi, ahi, 0x5140), ba3 = __byte_perm(bhi, ahi, 0x7362);
+                    uint4 *o = reinterpret_cast<uint4 *>(row);
+                    o[0] = make_uint4(__byte_perm(rg0, ba0, 0x5410), __byte_perm(rg0, ba0, 0x7632), __byte_perm(rg1, ba1, 0x5410),
+                                      __byte_perm(rg1, ba1, 0x7632));
+                    o[1] = make_uint4(__byte_perm(rg2, ba2, 0x5410), __byte_perm(rg2, ba2, 0x7632), __byte_perm(rg3, ba3, 0x5410),
+                                      __byte_perm(rg3, ba3, 0x7632));
+                }
+            } else if (act) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) row[i * 4 + c] = (uint8_t)px[i];
+            }
         }
     }
 }
@@ -138,8 +228,8 @@ __device__ __forceinline__ void load_nonce(const DctParams &p, int n, uint32_t (
     }
 }
 
-// One SHA-256 stream living in a lane's slot: `carry` words wait at [base+15-carry, base+15), `fresh` new words
-// were just written at [base+15, base+15+fresh). Compress every full 16-word block, slide the rest down.
+// One SHA-256 stream living in a lane's slot: `carry` words wait at [base+16-carry, base+16), `fresh` new words
+// were just written at [base+16, base+16+fresh). Compress every full 16-word block, slide the rest down.
 struct ShaStream {
     uint32_t H[8];
     int base;
@@ -165,7 +255,7 @@ __device__ __forceinline__ void write_padding(uint32_t *my, ShaStream &s) {
     int tot = n + 3;                      // 0x80 word + 64-bit length
     tot = (tot + 15) & ~15;               // 16 or 32
     const int fresh = tot - n;
-    uint32_t *dst = my + s.base + CARRY;
+    uint32_t *dst = my + s.base + CA;
     dst[0] = 0x00000080u;
     for (int i = 1; i < fresh - 2; ++i) dst[i] = 0u;
     const unsigned long long bits = (unsigned long long)s.total_words * 32ull;
@@ -174,18 +264,29 @@ __device__ __forceinline__ void write_padding(uint32_t *my, ShaStream &s) {
     s.fresh = fresh;
 }
 
+// `VA` = alignment (in words) every quantity of this stream is a multiple of: the window start, carry and fresh.
+template <int VA>
 __device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s) {
     int cnt = s.carry + s.fresh;
-    int ptr = s.base + CARRY - s.carry;
+    int ptr = s.base + CA - s.carry;
     while (cnt >= 16) {
         uint32_t w[16];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) w[i] = bswap32(my[ptr + i]);
+        for (int i = 0; i < 16; i += VA) {
+            uint32_t x[VA];
+            vec_load<VA>(my + ptr + i, x);
+#pragma unroll
+            for (int t = 0; t < VA; ++t) w[i + t] = bswap32(x[t]);
+        }
+#if !defined(FEDS_SHA_ROLLED) || FEDS_SHA_ROLLED
+        sha256_compress_rolled(s.H, w);
+#else
         sha256_compress(s.H, w);
+#endif
         ptr += 16;
         cnt -= 16;
     }
-    const int dst = s.base + CARRY - cnt;
+    const int dst = s.base + CA - cnt;
     if (dst != ptr)
         for (int i = 0; i < cnt; ++i) my[dst + i] = my[ptr + i];  // dst <= ptr: ascending copy is safe
     s.carry = cnt;
@@ -206,30 +307,87 @@ __device__ __forceinline__ void load_aes_tables(uint32_t *sT) {
     __syncthreads();
 }
 
-// Sequential CTR keystream along one private run: word `wi` (absolute 32-bit word index in the image's private
-// stream) -> keystream word; a new AES block is computed only when wi crosses a 16-byte boundary.
+// Sequential CTR keystream along one private run: V words starting at word `wi` (absolute 32-bit word index in
+// the image's private stream, a multiple of V); a new AES block is computed only when a 16-byte boundary is crossed.
 struct Keystream {
     uint32_t ks[4];
     unsigned long long blk;
 };
-__device__ __forceinline__ uint32_t keystream_word(Keystream &K, const uint32_t *sT, const uint32_t *rk, const uint32_t (&nonce)[4],
-                                                   unsigned long long wi) {
+template <int V>
+__device__ __forceinline__ void keystream_words(Keystream &K, const uint32_t *sT, const uint32_t *rk, const uint32_t (&nonce)[4],
+                                                unsigned long long wi, uint32_t (&out)[V]) {
     const unsigned long long blk = wi >> 2;
-    if (blk != K.blk) {
+    if (V == 4 || blk != K.blk) {
         ctr_block(nonce, blk, K.ks);
         aes128_encrypt(sT, rk, K.ks);
         K.blk = blk;
     }
-    const int sel = (int)(wi & 3);
-    return sel == 0 ? K.ks[0] : sel == 1 ? K.ks[1] : sel == 2 ? K.ks[2] : K.ks[3];
+    if (V == 4) {
+#pragma unroll
+        for (int t = 0; t < V; ++t) out[t] = K.ks[t];
+    } else if (V == 2) {
+        const bool up = (wi & 2) != 0;
+        out[0] = up ? K.ks[2] : K.ks[0];
+        out[1 % V] = up ? K.ks[3] : K.ks[1];
+    } else {
+        const int sel = (int)(wi & 3);
+        out[0] = sel == 0 ? K.ks[0] : sel == 1 ? K.ks[1] : sel == 2 ? K.ks[2] : K.ks[3];
+    }
+}
+
+// V == 1 only: the warp moves every active lane's public (Q words) and private (P words) run between the lanes' slots
+// and global memory with coalesced 32-bit accesses. pd / vd: this lane's run pointers for the phase (0 = inactive).
+template <bool TO_GLOBAL>
+__device__ __forceinline__ void warp_copy_runs(uint32_t *wslots, int stride, int P, int Q, unsigned long long pd, unsigned long long vd) {
+    const int lane = threadIdx.x & 31;
+#pragma unroll 1
+    for (int l0 = 0; l0 < 32; l0 += 4) {
+        unsigned long long pq[4], vq[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { pq[i] = __shfl_sync(0xffffffffu, pd, l0 + i); vq[i] = __shfl_sync(0xffffffffu, vd, l0 + i); }
+        if (TO_GLOBAL) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (vq[i] == 0ull) continue;
+                const uint32_t *src = wslots + (l0 + i) * stride;
+                uint32_t *dq = reinterpret_cast<uint32_t *>(pq[i]);
+                uint32_t *dp = reinterpret_cast<uint32_t *>(vq[i]);
+                if (lane < Q) dq[lane] = src[2 * CA + P + lane];
+                if (lane + 32 < Q) dq[lane + 32] = src[2 * CA + P + lane + 32];
+                if (lane < P) dp[lane] = src[CA + lane];
+                if (lane + 32 < P) dp[lane + 32] = src[CA + lane + 32];
+            }
+        } else {
+            uint32_t t[4][4];  // all loads of four runs are issued before the first store: one latency, not sixteen
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const bool on = vq[i] != 0ull;
+                const uint32_t *sq = reinterpret_cast<const uint32_t *>(pq[i]);
+                const uint32_t *sp = reinterpret_cast<const uint32_t *>(vq[i]);
+                t[i][0] = (on && lane < Q) ? __ldg(sq + lane) : 0u;
+                t[i][1] = (on && lane + 32 < Q) ? __ldg(sq + lane + 32) : 0u;
+                t[i][2] = (on && lane < P) ? __ldg(sp + lane) : 0u;
+                t[i][3] = (on && lane + 32 < P) ? __ldg(sp + lane + 32) : 0u;
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (vq[i] == 0ull) continue;
+                uint32_t *dst = wslots + (l0 + i) * stride;
+                if (lane < Q) dst[2 * CA + P + lane] = t[i][0];
+                if (lane + 32 < Q) dst[2 * CA + P + lane + 32] = t[i][1];
+                if (lane < P) dst[CA + lane] = t[i][2];
+                if (lane + 32 < P) dst[CA + lane + 32] = t[i][3];
+            }
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
 // fragment: steps 1-5
 // ------------------------------------------------------------------------------------------------------------
-template <int C, bool DIGEST>
-__global__ void __launch_bounds__(DCT_THREADS, 4) fragment_dct_kernel(const __grid_constant__ DctParams p) {
-    extern __shared__ uint32_t smem[];
+template <int C, int V, bool DIGEST>
+__global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_kernel(const __grid_constant__ DctParams p) {
+    extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
     load_aes_tables(sT);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -249,53 +407,61 @@ __global__ void __launch_bounds__(DCT_THREADS, 4) fragment_dct_kernel(const __gr
     // final phase the private stream's padding may spill into the (then finished) public region.
     ShaStream cur, oth;
     sha256_init(cur.H); sha256_init(oth.H);
-    cur.base = CARRY + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
+    cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
     oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
     Keystream K;
     K.blk = ~0ull;
     const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
+    uint32_t *mp = my + CA;      // private words of the current block, indexed by z
+    uint32_t *mq = my + 2 * CA;  // public words of the current block, indexed by z (z >= P)
 
+#pragma unroll 1
     for (int s = 0; s <= G_BLOCKS; ++s) {
         if (s < G_BLOCKS) {
             const bool act = s < L.nblk;
+            uint32_t *pq = pub_dst + (size_t)s * Q - P;  // public run of this block, indexed by z
+            uint32_t *pv = priv_dst + (size_t)s * P;      // private run of this block, indexed by z
             if (act) {
                 float v[64];
                 load_block<C>(img, p.w, 8 * L.br, 8 * (L.g * G_BLOCKS + s), L.c, v);
                 dct8x8(v);
-                uint32_t *mp = my + CARRY;      // private words: [15, 15+P), indexed by z
-                uint32_t *mq = my + 2 * CARRY;  // public words: region base (15+P) + 15 + (z-P) = 30 + z, indexed by z
 #pragma unroll
-                for (int z = 0; z < 64; ++z) {
-                    const uint32_t bits = __float_as_uint(v[ZZ.pos[z]]);
-                    if (z <= k) mp[z] = bits; else mq[z] = bits;
+                for (int g = 0; g < 64; g += V) {
+                    uint32_t x[V];
+#pragma unroll
+                    for (int t = 0; t < V; ++t) x[t] = __float_as_uint(v[ZZ.pos[g + t]]);
+                    if (g < P) {
+                        vec_store<V>(mp + g, x);   // plaintext; encrypted in place below
+                    } else {
+                        if (DIGEST || V == 1) vec_store<V>(mq + g, x);
+                        if (V > 1) vec_store<V>(pq + g, x);
+                    }
                 }
                 const unsigned long long w0 = priv_word0 + (unsigned long long)s * P;
-                for (int j = 0; j < P; ++j) mp[j] ^= keystream_word(K, sT, p.rk, nonce, w0 + j);
+#pragma unroll 1
+                for (int j = 0; j < P; j += V) {
+                    uint32_t ks[V], x[V];
+                    keystream_words<V>(K, sT, p.rk, nonce, w0 + j, ks);
+                    vec_load<V>(mp + j, x);
+#pragma unroll
+                    for (int t = 0; t < V; ++t) x[t] ^= ks[t];
+                    if (DIGEST || V == 1) vec_store<V>(mp + j, x);
+                    if (V > 1) vec_store<V>(pv + j, x);
+                }
             }
-            __syncwarp();
-            // the warp copies every lane's two runs out, coalesced
-            const unsigned long long pd = act ? reinterpret_cast<unsigned long long>(pub_dst + (size_t)s * Q) : 0ull;
-            const unsigned long long vd = act ? reinterpret_cast<unsigned long long>(priv_dst + (size_t)s * P) : 0ull;
-            for (int l = 0; l < 32; ++l) {
-                const unsigned long long pdl = __shfl_sync(0xffffffffu, pd, l);
-                const unsigned long long vdl = __shfl_sync(0xffffffffu, vd, l);
-                if (pdl == 0ull) continue;
-                const uint32_t *src = wslots + l * p.slot_stride;
-                uint32_t *dq = reinterpret_cast<uint32_t *>(pdl);
-                uint32_t *dp = reinterpret_cast<uint32_t *>(vdl);
-                if (lane < Q) dq[lane] = src[2 * CARRY + P + lane];
-                if (lane + 32 < Q) dq[lane + 32] = src[2 * CARRY + P + lane + 32];
-                if (lane < P) dp[lane] = src[CARRY + lane];
-                if (lane + 32 < P) dp[lane + 32] = src[CARRY + lane + 32];
+            if (V == 1) {
+                __syncwarp();
+                warp_copy_runs<true>(wslots, p.slot_stride, P, Q, act ? reinterpret_cast<unsigned long long>(pq + P) : 0ull,
+                                     act ? reinterpret_cast<unsigned long long>(pv) : 0ull);
+                __syncwarp();
             }
-            __syncwarp();
             if (DIGEST) { cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0; }
         }
         if (DIGEST) {
 #pragma unroll 1
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb(my, cur);
+                absorb<V>(my, cur);
                 swap_streams(cur, oth);
             }
         }
@@ -310,9 +476,9 @@ __global__ void __launch_bounds__(DCT_THREADS, 4) fragment_dct_kernel(const __gr
 // ------------------------------------------------------------------------------------------------------------
 // defragment: steps 6-8 (+ recomputation of the leaf digests of the fragments as received when VERIFY)
 // ------------------------------------------------------------------------------------------------------------
-template <int C, bool VERIFY>
-__global__ void __launch_bounds__(DCT_THREADS, 4) defragment_dct_kernel(const __grid_constant__ DctParams p) {
-    extern __shared__ uint32_t smem[];
+template <int C, int V, bool VERIFY>
+__global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_kernel(const __grid_constant__ DctParams p) {
+    extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
     load_aes_tables(sT);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -328,58 +494,77 @@ __global__ void __launch_bounds__(DCT_THREADS, 4) defragment_dct_kernel(const __
     uint32_t nonce[4];
     load_nonce(p, L.n, nonce);
 
-    // cur = public stream, oth = private stream (swapped twice per phase). The public stream goes first so that in the
-    // final phase the private stream's padding may spill into the (then finished) public region.
     ShaStream cur, oth;
     sha256_init(cur.H); sha256_init(oth.H);
-    cur.base = CARRY + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
+    cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
     oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
     Keystream K;
     K.blk = ~0ull;
     const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
+    uint32_t *mp = my + CA;
+    uint32_t *mq = my + 2 * CA;
 
+#pragma unroll 1
     for (int s = 0; s <= G_BLOCKS; ++s) {
         const bool act = s < L.nblk;
+        const uint32_t *pq = pub_src + (size_t)s * Q - P;  // indexed by z
+        const uint32_t *pv = priv_src + (size_t)s * P;
         if (s < G_BLOCKS) {
-            // the warp copies every lane's two runs in, coalesced
-            const unsigned long long pd = act ? reinterpret_cast<unsigned long long>(pub_src + (size_t)s * Q) : 0ull;
-            const unsigned long long vd = act ? reinterpret_cast<unsigned long long>(priv_src + (size_t)s * P) : 0ull;
-            for (int l = 0; l < 32; ++l) {
-                const unsigned long long pdl = __shfl_sync(0xffffffffu, pd, l);
-                const unsigned long long vdl = __shfl_sync(0xffffffffu, vd, l);
-                if (vdl == 0ull) continue;
-                uint32_t *dst = wslots + l * p.slot_stride;
-                const uint32_t *sq = reinterpret_cast<const uint32_t *>(pdl);
-                const uint32_t *sp = reinterpret_cast<const uint32_t *>(vdl);
-                if (lane < Q) dst[2 * CARRY + P + lane] = __ldg(sq + lane);
-                if (lane + 32 < Q) dst[2 * CARRY + P + lane + 32] = __ldg(sq + lane + 32);
-                if (lane < P) dst[CARRY + lane] = __ldg(sp + lane);
-                if (lane + 32 < P) dst[CARRY + lane + 32] = __ldg(sp + lane + 32);
+            if (V == 1) {
+                warp_copy_runs<false>(wslots, p.slot_stride, P, Q, act ? reinterpret_cast<unsigned long long>(pq + P) : 0ull,
+                                      act ? reinterpret_cast<unsigned long long>(pv) : 0ull);
+                __syncwarp();
+            } else if (act) {
+                // each lane pulls its own runs: all loads first, then the stores into the slot
+#pragma unroll
+                for (int g0 = 0; g0 < 64; g0 += 8 * V) {
+                    uint32_t x[8][V];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int g = g0 + i * V;
+                        if (g < P) vec_load_global<V>(pv + g, x[i]); else vec_load_global<V>(pq + g, x[i]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const int g = g0 + i * V;
+                        vec_store<V>(g < P ? mp + g : mq + g, x[i]);
+                    }
+                }
             }
-            __syncwarp();
             if (VERIFY) { cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0; }
         }
         if (VERIFY) {
 #pragma unroll 1
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb(my, cur);  // hashes the bytes as received (ciphertext / public coefficients); keeps [base+15, ..) intact
+                absorb<V>(my, cur);  // hashes the bytes as received; leaves [base+16, ..) of the current block intact
                 swap_streams(cur, oth);
             }
         }
         if (s < G_BLOCKS) {
+            float v[64];
             if (act) {
-                uint32_t *mp = my + CARRY;
-                const uint32_t *mq = my + 2 * CARRY;
                 const unsigned long long w0 = priv_word0 + (unsigned long long)s * P;
-                for (int j = 0; j < P; ++j) mp[j] ^= keystream_word(K, sT, p.rk, nonce, w0 + j);
-                float v[64];
+#pragma unroll 1
+                for (int j = 0; j < P; j += V) {
+                    uint32_t ks[V], x[V];
+                    keystream_words<V>(K, sT, p.rk, nonce, w0 + j, ks);
+                    vec_load<V>(mp + j, x);
 #pragma unroll
-                for (int z = 0; z < 64; ++z) v[ZZ.pos[z]] = __uint_as_float(z <= k ? mp[z] : mq[z]);
+                    for (int t = 0; t < V; ++t) x[t] ^= ks[t];
+                    vec_store<V>(mp + j, x);
+                }
+#pragma unroll
+                for (int g = 0; g < 64; g += V) {
+                    uint32_t x[V];
+                    vec_load<V>(g < P ? mp + g : mq + g, x);
+#pragma unroll
+                    for (int t = 0; t < V; ++t) v[ZZ.pos[g + t]] = __uint_as_float(x[t]);
+                }
                 idct8x8(v);
-                store_block<C>(img, p.w, 8 * L.br, 8 * (L.g * G_BLOCKS + s), L.c, v);
             }
-            __syncwarp();  // the next phase's copy-in overwrites the slots
+            store_block<C>(img, p.w, 8 * L.br, 8 * (L.g * G_BLOCKS + s), L.c, act, v);
+            if (V == 1) __syncwarp();  // the next phase's copy-in overwrites the slots
         }
     }
     if (VERIFY && L.valid) {
