@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("FEDS_LIB_PATH") or os.path.join(HERE, "libfeds.so")
 SOURCES = ["feds_api.cu"]
-HEADERS = ["feds_device.cuh", "feds_dct.cuh", "feds_hash.cuh", "feds_dwt.cuh", os.path.join("..", "..", "include", "feds.h")]
+HEADERS = ["feds_device.cuh", "feds_dct.cuh", "feds_hash.cuh", "feds_dwt.cuh", "feds_peaks.cu", os.path.join("..", "..", "include", "feds.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -49,7 +49,23 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if verbose:
         sys.stderr.write(res.stderr)
     os.replace(tmp, LIB)
+    build_peaks(nvcc)
     return LIB
+
+
+PEAKS = os.path.join(HERE, "feds_peaks")
+
+
+def build_peaks(nvcc=None) -> str:
+    """The small stand-alone tool that measures this GPU's SHA-256 integer ceiling (bench.py's ALU-roofline context)."""
+    nvcc = nvcc or os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "--expt-relaxed-constexpr",
+           "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64", "-o", PEAKS, os.path.join(CSRC, "feds_peaks.cu")]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed on feds_peaks.cu")
+    return PEAKS
 
 
 if __name__ == "__main__":

@@ -122,6 +122,7 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.leaves_per_image = (unsigned)c * p.nbr * p.nlr;
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
     p.slot_stride = dct_slot_words(k);
+    p.one = 1u;
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);

@@ -43,6 +43,7 @@ struct DctParams {
     unsigned leaves_per_image;  // C * nbr * nlr
     unsigned long long total_leaves;
     int slot_stride;  // words per lane slot
+    uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
 };
 
 // Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:
@@ -266,7 +267,7 @@ __device__ __forceinline__ void write_padding(uint32_t *my, ShaStream &s) {
 
 // `VA` = alignment (in words) every quantity of this stream is a multiple of: the window start, carry and fresh.
 template <int VA>
-__device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s) {
+__device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s, const uint32_t one) {
     int cnt = s.carry + s.fresh;
     int ptr = s.base + CA - s.carry;
     while (cnt >= 16) {
@@ -278,7 +279,10 @@ __device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s) {
 #pragma unroll
             for (int t = 0; t < VA; ++t) w[i + t] = bswap32(x[t]);
         }
-#if !defined(FEDS_SHA_ROLLED) || FEDS_SHA_ROLLED
+#if !defined(FEDS_SHA_FMA_ADDS) || FEDS_SHA_FMA_ADDS  // default: +6 % on B200 (ALU pipe is the binding unit, FMA pipe idles)
+        sha256_compress_rolled_fma(s.H, w, one);
+#elif !defined(FEDS_SHA_ROLLED) || FEDS_SHA_ROLLED
+        (void)one;
         sha256_compress_rolled(s.H, w);
 #else
         sha256_compress(s.H, w);
@@ -461,7 +465,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
 #pragma unroll 1
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb<V>(my, cur);
+                absorb<V>(my, cur, p.one);
                 swap_streams(cur, oth);
             }
         }
@@ -537,7 +541,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
 #pragma unroll 1
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb<V>(my, cur);  // hashes the bytes as received; leaves [base+16, ..) of the current block intact
+                absorb<V>(my, cur, p.one);  // hashes the bytes as received; leaves [base+16, ..) of the current block intact
                 swap_streams(cur, oth);
             }
         }

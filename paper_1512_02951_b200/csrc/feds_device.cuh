@@ -107,6 +107,41 @@ FEDS_HD void sha256_compress_rolled(uint32_t (&H)[8], uint32_t (&w)[16]) {
     H[0] += a; H[1] += b; H[2] += c; H[3] += d; H[4] += e; H[5] += f; H[6] += g; H[7] += h;
 }
 
+// Variant whose 32-bit additions are issued as IMAD (x * one + y, `one` = 1 known only at run time) so that they
+// execute on the FMA pipe and leave the ALU pipe to the shifts and logic ops that can run nowhere else.
+FEDS_HD uint32_t add_fma(uint32_t x, uint32_t y, uint32_t one) { return x * one + y; }
+FEDS_HD void sha256_compress_rolled_fma(uint32_t (&H)[8], uint32_t (&w)[16], const uint32_t one) {
+#ifndef __CUDA_ARCH__
+    constexpr uint32_t K[64] = {FEDS_SHA256_K_LIST};
+#endif
+    uint32_t a = H[0], b = H[1], c = H[2], d = H[3], e = H[4], f = H[5], g = H[6], h = H[7];
+#pragma unroll 1
+    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            if (i > 0) {
+                const uint32_t w15 = w[(j + 1) & 15], w2 = w[(j + 14) & 15];
+                const uint32_t s0 = rotr32(w15, 7) ^ rotr32(w15, 18) ^ (w15 >> 3);
+                const uint32_t s1 = rotr32(w2, 17) ^ rotr32(w2, 19) ^ (w2 >> 10);
+                w[j] = add_fma(add_fma(w[j], s0, one), add_fma(w[(j + 9) & 15], s1, one), one);
+            }
+#ifdef __CUDA_ARCH__
+            const uint32_t kt = c_sha256_k[16 * i + j];
+#else
+            const uint32_t kt = K[16 * i + j];
+#endif
+            const uint32_t S1 = rotr32(e, 6) ^ rotr32(e, 11) ^ rotr32(e, 25);
+            const uint32_t ch = (e & f) ^ (~e & g);
+            const uint32_t hk = add_fma(add_fma(h, kt, one), w[j], one);
+            const uint32_t T1 = add_fma(add_fma(S1, ch, one), hk, one);
+            const uint32_t S0 = rotr32(a, 2) ^ rotr32(a, 13) ^ rotr32(a, 22);
+            const uint32_t maj = (a & b) ^ (a & c) ^ (b & c);
+            h = g; g = f; f = e; e = add_fma(d, T1, one); d = c; c = b; b = a; a = add_fma(add_fma(S0, maj, one), T1, one);
+        }
+    }
+    H[0] += a; H[1] += b; H[2] += c; H[3] += d; H[4] += e; H[5] += f; H[6] += g; H[7] += h;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // AES-128 (FIPS-197) with one-lookup-per-byte round tables. State = 4 column words, byte r of a word = row r
 // (little-endian view of the FIPS-197 input bytes in[r + 4c]).
