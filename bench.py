@@ -37,6 +37,16 @@ WORKLOADS = {
 }
 
 
+def tree_launch_count(n_leaves):
+    """Launches run_tree() makes for one tree shape: one merkle_level_kernel per level wider than 4096 digests, then one
+    merkle_tail_kernel (up to three levels in one CTA per tree)."""
+    t = 0
+    while n_leaves > 4096:
+        n_leaves = (n_leaves + 15) // 16
+        t += 1
+    return t + (1 if n_leaves > 1 else 0)
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -201,11 +211,7 @@ def main():
         d_out = torch.empty_like(d_imgs)
         batch = B.DctBatch(n, w, h, c, kl, device=dev)
         nl = c * (h // 8) * ((w // 8 + 7) // 8)
-        tree_launches = 0
-        m = nl
-        while m > 1:
-            m = (m + 15) // 16
-            tree_launches += 1
+        tree_launches = tree_launch_count(nl)
         per_step_launches = (1 + tree_launches) + (1 + tree_launches + 1)
 
         def step(record=False):
@@ -227,13 +233,10 @@ def main():
         ws = torch.empty(B.workspace_bytes(w, h, c, kl, True), dtype=torch.uint8, device=dev)
         state = {}
 
-        def tl(nbytes):
-            m, t = (nbytes + 2047) // 2048, 0
-            while m > 1:
-                m = (m + 15) // 16
-                t += 1
-            return t
-        per_dig = 2 + tl(B.dwt_private_bytes(w, h, c, kl)) + tl(B.dwt_public_bytes(w, h, c, kl))
+        def wide(nbytes):   # merkle_level_kernel launches of one tree; both tops share one merkle_tail_kernel launch
+            nl_ = (nbytes + 2047) // 2048
+            return tree_launch_count(nl_) - (1 if nl_ > 1 else 0)
+        per_dig = 1 + wide(B.dwt_private_bytes(w, h, c, kl)) + wide(B.dwt_public_bytes(w, h, c, kl)) + 1
         per_step_launches = (kl + 1 + per_dig) + (per_dig + 1 + 1 + kl)
 
         def step(record=False):

@@ -63,27 +63,63 @@ void nonce_to_be(const uint8_t nonce[16], uint32_t out[4]) {
 
 // Reduce level-0 digests [tree][n0][32] (tree stride = n0*32) to roots written at roots + tree*root_stride.
 // `scratch` holds the intermediate levels. n_trees trees of identical shape.
-feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
-                     int skip_odd, cudaStream_t stream) {
-    unsigned n[40];
-    const int L = tree_levels(n0, n);
-    const uint8_t *in = level0;
-    uint8_t *sc = scratch;
-    for (int i = 0; i + 1 < L; ++i) {
-        MerkleLevelParams mp;
-        mp.in = in;
-        mp.n_in = n[i];
-        mp.n_out = n[i + 1];
-        mp.n_trees = n_trees;
-        mp.in_tree_stride = (size_t)n[i] * 32;
-        mp.odd_trees_only_if_nonempty = skip_odd;
-        if (n[i + 1] == 1) { mp.out = roots; mp.out_tree_stride = root_stride; }
-        else { mp.out = sc; mp.out_tree_stride = (size_t)n[i + 1] * 32; sc += (size_t)n_trees * n[i + 1] * 32; }
-        const unsigned long long threads = (unsigned long long)n_trees * n[i + 1];
+// wide levels of n_trees equal trees: one thread per node until at most TAIL_MAX_IN digests per tree remain
+feds_status reduce_wide(const uint8_t *&in, unsigned &n, unsigned n_trees, uint8_t *&sc, int skip_odd, cudaStream_t stream) {
+    MerkleLevelParams mp{};
+    mp.n_trees = n_trees;
+    mp.odd_trees_only_if_nonempty = skip_odd;
+    mp.one = 1u;
+    while (n > TAIL_MAX_IN) {
+        const unsigned m = (n + FANOUT - 1) / FANOUT;
+        mp.in = in; mp.n_in = n; mp.n_out = m; mp.in_tree_stride = (size_t)n * 32;
+        mp.out = sc; mp.out_tree_stride = (size_t)m * 32;
+        const unsigned long long threads = (unsigned long long)n_trees * m;
         merkle_level_kernel<<<(unsigned)((threads + HASH_THREADS - 1) / HASH_THREADS), HASH_THREADS, 0, stream>>>(mp);
         FEDS_LAUNCH_CHECK();
-        in = mp.out;
+        in = sc;
+        sc += (size_t)n_trees * m * 32;
+        n = m;
     }
+    return FEDS_OK;
+}
+
+feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
+                     int skip_odd, cudaStream_t stream) {
+    const uint8_t *in = level0;
+    uint8_t *sc = scratch;
+    unsigned n = n0;
+    feds_status st = reduce_wide(in, n, n_trees, sc, skip_odd, stream);
+    if (st != FEDS_OK) return st;
+    if (n > 1) {  // the top (<= 4096 digests per tree): one CTA per tree, up to three levels in one launch
+        MerkleLevelParams mp{};
+        mp.n_trees = n_trees; mp.odd_trees_only_if_nonempty = skip_odd; mp.one = 1u;
+        mp.in = in; mp.n_in = n; mp.n_out = 1; mp.in_tree_stride = (size_t)n * 32;
+        mp.out = roots; mp.out_tree_stride = root_stride;
+        merkle_tail_kernel<<<n_trees, TAIL_THREADS, 0, stream>>>(mp);
+        FEDS_LAUNCH_CHECK();
+    }
+    return FEDS_OK;
+}
+
+// two single trees of different shapes (DWT private / public): wide levels separately, both tops in one launch
+feds_status run_two_trees(const uint8_t *l0a, unsigned na, uint8_t *sca, uint8_t *roota, const uint8_t *l0b, unsigned nb, uint8_t *scb,
+                          uint8_t *rootb, cudaStream_t stream) {
+    const uint8_t *ina = l0a, *inb = l0b;
+    feds_status st = reduce_wide(ina, na, 1, sca, 0, stream);
+    if (st != FEDS_OK) return st;
+    st = reduce_wide(inb, nb, 1, scb, 0, stream);
+    if (st != FEDS_OK) return st;
+    if (na <= 1 && nb <= 1) return FEDS_OK;  // one-leaf trees: the leaf kernel already wrote the roots
+    MerkleLevelParams mp{};
+    mp.one = 1u; mp.n_out = 1;
+    unsigned ctas = 0;
+    if (na > 1) { mp.n_trees = 1; mp.in = ina; mp.n_in = na; mp.in_tree_stride = 0; mp.out = roota; mp.out_tree_stride = 0; ctas = 1; }
+    if (nb > 1) {
+        if (ctas == 0) { mp.n_trees = 1; mp.in = inb; mp.n_in = nb; mp.out = rootb; ctas = 1; }
+        else { mp.in2 = inb; mp.n_in2 = nb; mp.out2 = rootb; ctas = 2; }
+    }
+    merkle_tail_kernel<<<ctas, TAIL_THREADS, 0, stream>>>(mp);
+    FEDS_LAUNCH_CHECK();
     return FEDS_OK;
 }
 
@@ -289,23 +325,20 @@ size_t dwt_level_off_elems(int w, int h, int L, int l) {  // elements before lev
 
 feds_status dwt_digests(const uint8_t *d_private, const uint8_t *d_public, const DwtPlan &pl, uint8_t *tree_ws, uint8_t *roots,
                         cudaStream_t stream) {
-    const uint8_t *streams[2] = {d_private, d_public};
-    const size_t nbytes[2] = {pl.priv_b, pl.pub_b};
     const unsigned nls[2] = {pl.priv_nl, pl.pub_nl};
     uint8_t *ws[2] = {tree_ws, tree_ws + round_up(pl.priv_tree, 256)};
+    StreamLeavesParams sp;
+    sp.data[0] = d_private; sp.data[1] = d_public;
+    sp.n_bytes[0] = pl.priv_b; sp.n_bytes[1] = pl.pub_b;
+    sp.one = 1u;
     for (int f = 0; f < 2; ++f) {
-        StreamLeavesParams sp;
-        sp.data = streams[f]; sp.stream_stride = 0; sp.n_bytes = nbytes[f]; sp.n_leaves = nls[f]; sp.n_streams = 1;
-        sp.out = nls[f] > 1 ? ws[f] : roots + 32 * f;
-        sp.out_stream_stride = 0;
-        stream_leaves_kernel<<<(nls[f] + HASH_THREADS - 1) / HASH_THREADS, HASH_THREADS, 0, stream>>>(sp);
-        FEDS_LAUNCH_CHECK();
-        if (nls[f] > 1) {
-            feds_status st = run_tree(ws[f], nls[f], 1, ws[f] + (size_t)nls[f] * 32, roots + 32 * f, 64, 0, stream);
-            if (st != FEDS_OK) return st;
-        }
+        sp.n_leaves[f] = nls[f];
+        sp.out[f] = nls[f] > 1 ? ws[f] : roots + 32 * f;  // a one-leaf fragment's root is its leaf digest
     }
-    return FEDS_OK;
+    const unsigned total = nls[0] + nls[1];
+    stream_leaves_kernel<<<(total + HASH_THREADS - 1) / HASH_THREADS, HASH_THREADS, 0, stream>>>(sp);
+    FEDS_LAUNCH_CHECK();
+    return run_two_trees(ws[0], nls[0], ws[0] + (size_t)nls[0] * 32, roots, ws[1], nls[1], ws[1] + (size_t)nls[1] * 32, roots + 32, stream);
 }
 
 }  // namespace

@@ -4,6 +4,8 @@
 // with x[N] = x[N-2], d[-1] = d[0] (P:755-762 in the DESIGN.md A12/A14 reading); rows then columns forward
 // (P:812), columns then rows inverse. A CTA transforms one tile with its halo staged in shared memory; integer
 // arithmetic makes the result independent of the tiling. Arithmetic shifts are floors (toward -inf).
+// Global traffic is vectorised wherever the addresses allow (aligned 4-byte loads of 4 pixels / 2 coefficients,
+// 8/16-byte stores of 4/8/16 outputs); out-of-range or misaligned pieces fall back to mirrored scalar accesses.
 #pragma once
 #include "feds_device.cuh"
 
@@ -38,6 +40,9 @@ struct DwtLevelParams {
     size_t pub_image_stride, pub_chan_stride, level_off;
 };
 
+__device__ __forceinline__ bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
+__device__ __forceinline__ uint32_t pack16(int a, int b) { return ((uint32_t)a & 0xffffu) | ((uint32_t)b << 16); }
+
 // ------------------------------------------------------------------------------------------------------------
 // forward level
 // ------------------------------------------------------------------------------------------------------------
@@ -55,14 +60,49 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_fwd_level_kernel(const __grid
     const int bw = p.cw >> 1, bh = p.ch >> 1;
     const int tid = threadIdx.x;
 
-    // stage A: input tile with halo (mirrored at the borders)
-    for (int i = tid; i < IR * IC; i += DWT_THREADS) {
-        const int ly = i / IC, lx = i % IC;
-        const int y = mirror_idx(2 * ty0 - 2 + ly, p.ch), x = mirror_idx(2 * tx0 - 2 + lx, p.cw);
-        int v;
-        if (FIRST) v = (int)p.img_in[(size_t)n * p.image_stride + ((size_t)y * p.img_w + x) * p.C + c] - 128;
-        else v = p.ll_in[(size_t)plane * p.ll_in_plane_stride + (size_t)y * p.cw + x];
-        sIn[ly][lx] = (int16_t)v;
+    // stage A: input tile with halo (mirrored at the borders); local column lx <-> x = 2*tx0 - 2 + lx
+    if (FIRST) {
+        const uint8_t *img = p.img_in + (size_t)n * p.image_stride;
+        if (p.C == 1 && (p.img_w & 3) == 0) {
+            constexpr int NW = (IC + 2 + 3) / 4 + 1;  // aligned 4-pixel words covering x in [2*tx0 - 4, 2*tx0 + 2*TW + 4)
+            for (int i = tid; i < IR * NW; i += DWT_THREADS) {
+                const int ly = i / NW, j = i % NW;
+                const int y = mirror_idx(2 * ty0 - 2 + ly, p.ch), xw = 2 * tx0 - 4 + 4 * j;
+                const uint8_t *row = img + (size_t)y * p.img_w;
+                uint32_t q;
+                if (xw >= 0 && xw + 3 < p.cw) q = __ldg(reinterpret_cast<const uint32_t *>(row + xw));
+                else q = (uint32_t)row[mirror_idx(xw, p.cw)] | ((uint32_t)row[mirror_idx(xw + 1, p.cw)] << 8) |
+                         ((uint32_t)row[mirror_idx(xw + 2, p.cw)] << 16) | ((uint32_t)row[mirror_idx(xw + 3, p.cw)] << 24);
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    const int lx = 4 * j - 2 + t;
+                    if (lx >= 0 && lx < IC) sIn[ly][lx] = (int16_t)((int)((q >> (8 * t)) & 0xffu) - 128);
+                }
+            }
+        } else {
+            for (int i = tid; i < IR * IC; i += DWT_THREADS) {
+                const int ly = i / IC, lx = i % IC;
+                const int y = mirror_idx(2 * ty0 - 2 + ly, p.ch), x = mirror_idx(2 * tx0 - 2 + lx, p.cw);
+                sIn[ly][lx] = (int16_t)((int)img[((size_t)y * p.img_w + x) * p.C + c] - 128);
+            }
+        }
+    } else {
+        const int16_t *pl = p.ll_in + (size_t)plane * p.ll_in_plane_stride;
+        constexpr int NP = (IC + 1) / 2;  // aligned coefficient pairs covering x in [2*tx0 - 2, 2*tx0 + 2*TW + 2)
+        for (int i = tid; i < IR * NP; i += DWT_THREADS) {
+            const int ly = i / NP, j = i % NP;
+            const int y = mirror_idx(2 * ty0 - 2 + ly, p.ch), x = 2 * tx0 - 2 + 2 * j;
+            const int16_t *row = pl + (size_t)y * p.cw;
+            int a, b;
+            if (x >= 0 && x + 1 < p.cw) {
+                const uint32_t q = __ldg(reinterpret_cast<const uint32_t *>(row + x));
+                a = (int16_t)(q & 0xffffu); b = (int16_t)(q >> 16);
+            } else {
+                a = row[mirror_idx(x, p.cw)]; b = row[mirror_idx(x + 1, p.cw)];
+            }
+            sIn[ly][2 * j] = (int16_t)a;
+            if (2 * j + 1 < IC) sIn[ly][2 * j + 1] = (int16_t)b;
+        }
     }
     __syncthreads();
     // stage B: horizontal predict, d[n] for n in [tx0-1, tx0+TW)
@@ -88,23 +128,37 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_fwd_level_kernel(const __grid
         sVd[r][q] = (int16_t)(b - ((a + e) >> 1));
     }
     __syncthreads();
-    // vertical update + stores: LL/HL get s, LH/HH get d
+    // vertical update + stores: LL/HL get s, LH/HH get d. One item = 4 adjacent columns of one row of one half.
     int16_t *llb = p.ll_band + (size_t)n * p.ll_band_image_stride + (size_t)c * p.ll_band_chan_stride;
     int16_t *pb = p.pub + (size_t)n * p.pub_image_stride + (size_t)c * p.pub_chan_stride + p.level_off;
     const size_t band = (size_t)bw * bh;
-    for (int i = tid; i < DWT_TH * 2 * DWT_TW; i += DWT_THREADS) {
-        const int r = i / (2 * DWT_TW), q = i % (2 * DWT_TW);  // m = ty0 + r
-        const int m = ty0 + r;
-        const bool high = q >= DWT_TW;
-        const int j = high ? q - DWT_TW : q;
-        const int nn = tx0 + j;
-        if (m >= bh || nn >= bw) continue;
-        const int x2m = high ? (int)sHd[2 * r + 2][j + 1] : (int)sHs[2 * r + 2][j];
-        const int dprev = sVd[r][q], dcur = sVd[r + 1][q];
-        const int s = x2m + ((dprev + dcur + 2) >> 2);
-        const size_t o = (size_t)m * bw + nn;
-        if (!high) { llb[o] = (int16_t)s; pb[1 * band + o] = (int16_t)dcur; }       // LL, LH
-        else { pb[0 * band + o] = (int16_t)s; pb[2 * band + o] = (int16_t)dcur; }   // HL, HH
+    const bool vec_ok = (bw & 3) == 0 && aligned8(llb) && aligned8(pb) && aligned8(pb + band) && aligned8(pb + 2 * band);
+    for (int i = tid; i < DWT_TH * 2 * (DWT_TW / 4); i += DWT_THREADS) {
+        const int r = i / (2 * (DWT_TW / 4)), rem = i % (2 * (DWT_TW / 4));
+        const bool high = rem >= DWT_TW / 4;
+        const int j0 = 4 * (high ? rem - DWT_TW / 4 : rem);
+        const int m = ty0 + r, nn0 = tx0 + j0;
+        if (m >= bh || nn0 >= bw) continue;
+        int sv[4], dv[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            const int j = j0 + t, q = high ? DWT_TW + j : j;
+            const int x2m = high ? (int)sHd[2 * r + 2][j + 1] : (int)sHs[2 * r + 2][j];
+            const int dprev = sVd[r][q], dcur = sVd[r + 1][q];
+            sv[t] = x2m + ((dprev + dcur + 2) >> 2);
+            dv[t] = dcur;
+        }
+        const size_t o = (size_t)m * bw + nn0;
+        int16_t *ps = high ? pb + 0 * band + o : llb + o;         // HL or LL
+        int16_t *pd = high ? pb + 2 * band + o : pb + 1 * band + o;  // HH or LH
+        if (vec_ok && nn0 + 3 < bw) {
+            *reinterpret_cast<uint2 *>(ps) = make_uint2(pack16(sv[0], sv[1]), pack16(sv[2], sv[3]));
+            *reinterpret_cast<uint2 *>(pd) = make_uint2(pack16(dv[0], dv[1]), pack16(dv[2], dv[3]));
+        } else {
+#pragma unroll
+            for (int t = 0; t < 4; ++t)
+                if (nn0 + t < bw) { ps[t] = (int16_t)sv[t]; pd[t] = (int16_t)dv[t]; }
+        }
     }
 }
 
@@ -114,10 +168,10 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_fwd_level_kernel(const __grid
 template <bool LAST>
 __global__ void __launch_bounds__(DWT_THREADS) dwt_inv_level_kernel(const __grid_constant__ DwtLevelParams p) {
     constexpr int SR = DWT_TH + 2, SC = DWT_TW + 2;  // subband rows m in [ty0-1, ty0+TH], cols n in [tx0-1, tx0+TW]
-    __shared__ int16_t sB[4][SR][SC + 1];            // 0 LL, 1 HL, 2 LH, 3 HH
-    __shared__ int16_t sL[2 * DWT_TH + 1][SC + 1];   // after vertical synthesis: low-horizontal half, rows 2ty0 .. 2ty0+2TH
-    __shared__ int16_t sH[2 * DWT_TH + 1][SC + 1];   // high-horizontal half
-    __shared__ int16_t sE[2 * DWT_TH][DWT_TW + 1];   // even output columns x[2n], n in [tx0, tx0+TW]
+    __shared__ int16_t sB[4][SR][SC + 2];            // 0 LL, 1 HL, 2 LH, 3 HH
+    __shared__ int16_t sL[2 * DWT_TH + 1][SC + 2];   // after vertical synthesis: low-horizontal half, rows 2ty0 .. 2ty0+2TH
+    __shared__ int16_t sH[2 * DWT_TH + 1][SC + 2];   // high-horizontal half
+    __shared__ int16_t sE[2 * DWT_TH][DWT_TW + 2];   // even output columns x[2n], n in [tx0, tx0+TW]
 
     const int plane = blockIdx.z;
     const int n = plane / p.C, c = plane % p.C;
@@ -128,19 +182,28 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_inv_level_kernel(const __grid
     const int16_t *pb = p.pub + (size_t)n * p.pub_image_stride + (size_t)c * p.pub_chan_stride + p.level_off;
     const size_t band = (size_t)bw * bh;
 
-    for (int i = tid; i < 4 * SR * SC; i += DWT_THREADS) {
-        const int b = i / (SR * SC), rem = i % (SR * SC), lr = rem / SC, lc = rem % SC;
-        // d[-1] = d[0] (mirror at the low end); beyond the high end values are never used: clamp
-        int m = ty0 - 1 + lr, nn = tx0 - 1 + lc;
-        m = min(max(m, 0), bh - 1);
-        nn = min(max(nn, 0), bw - 1);
-        const size_t o = (size_t)m * bw + nn;
-        int16_t v;
-        if (b == 0) v = llb[o];
-        else if (b == 1) v = pb[0 * band + o];
-        else if (b == 2) v = pb[1 * band + o];
-        else v = pb[2 * band + o];
-        sB[b][lr][lc] = v;
+    // load the four bands with their halo; aligned pairs cover columns nn in [tx0-2, tx0+TW+2); lc = nn - (tx0-1)
+    {
+        constexpr int NP = (SC + 2) / 2;
+        const bool pair_ok = (bw & 1) == 0 && (reinterpret_cast<uintptr_t>(llb) & 3u) == 0 && (reinterpret_cast<uintptr_t>(pb) & 3u) == 0 &&
+                             (band & 1) == 0;
+        for (int i = tid; i < 4 * SR * NP; i += DWT_THREADS) {
+            const int b = i / (SR * NP), rem = i % (SR * NP), lr = rem / NP, j = rem % NP;
+            const int m = min(max(ty0 - 1 + lr, 0), bh - 1);  // d[-1] = d[0]; rows beyond the end are never used
+            const int16_t *src = (b == 0) ? llb : (b == 1) ? pb : (b == 2) ? pb + band : pb + 2 * band;
+            src += (size_t)m * bw;
+            const int nn = tx0 - 2 + 2 * j;
+            int a, e;
+            if (pair_ok && nn >= 0 && nn + 1 < bw) {
+                const uint32_t q = __ldg(reinterpret_cast<const uint32_t *>(src + nn));
+                a = (int16_t)(q & 0xffffu); e = (int16_t)(q >> 16);
+            } else {
+                a = src[min(max(nn, 0), bw - 1)]; e = src[min(max(nn + 1, 0), bw - 1)];
+            }
+            const int lc = 2 * j - 1;
+            if (lc >= 0) sB[b][lr][lc] = (int16_t)a;
+            if (lc + 1 < SC) sB[b][lr][lc + 1] = (int16_t)e;
+        }
     }
     __syncthreads();
     // vertical synthesis, even rows x[2m], m in [ty0, ty0+TH] (local r = 0..TH), all SC columns, both halves
@@ -157,7 +220,7 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_inv_level_kernel(const __grid
         const int half = i / (DWT_TH * SC), rem = i % (DWT_TH * SC), r = rem / SC, lc = rem % SC;
         const int db = half ? 3 : 2;
         const int m = ty0 + r;
-        const int16_t(*S)[SC + 1] = half ? sH : sL;
+        const int16_t(*S)[SC + 2] = half ? sH : sL;
         const int a = S[2 * r][lc];
         const int e = (m + 1 < bh) ? (int)S[2 * r + 2][lc] : a;
         const int16_t x = (int16_t)((int)sB[db][r + 1][lc] + ((a + e) >> 1));
@@ -170,24 +233,49 @@ __global__ void __launch_bounds__(DWT_THREADS) dwt_inv_level_kernel(const __grid
         sE[ry][j] = (int16_t)((int)sL[ry][j + 1] - (((int)sH[ry][j] + (int)sH[ry][j + 1] + 2) >> 2));
     }
     __syncthreads();
-    // outputs: even and odd columns
-    for (int i = tid; i < 2 * DWT_TH * 2 * DWT_TW; i += DWT_THREADS) {
-        const int ry = i / (2 * DWT_TW), cx = i % (2 * DWT_TW);
-        const int y = 2 * ty0 + ry, x = 2 * tx0 + cx;
-        if (y >= p.ch || x >= p.cw) continue;
-        const int j = cx >> 1;
-        int v;
-        if ((cx & 1) == 0) v = sE[ry][j];
-        else {
+    // outputs: one item = 16 adjacent output columns (8 even + 8 odd) of one row
+    const bool vec_ok = LAST ? (p.C == 1 && (p.img_w & 15) == 0 && (reinterpret_cast<uintptr_t>(p.img_out) & 15u) == 0 && (p.image_stride & 15u) == 0)
+                             : ((p.cw & 7) == 0 && (reinterpret_cast<uintptr_t>(p.ll_out_plane) & 15u) == 0 && (p.ll_out_plane_stride & 7u) == 0);
+    for (int i = tid; i < 2 * DWT_TH * (2 * DWT_TW / 16); i += DWT_THREADS) {
+        const int ry = i / (2 * DWT_TW / 16), cx0 = 16 * (i % (2 * DWT_TW / 16));
+        const int y = 2 * ty0 + ry, x0 = 2 * tx0 + cx0;
+        if (y >= p.ch || x0 >= p.cw) continue;
+        int v[16];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+            const int j = (cx0 >> 1) + t;
             const int a = sE[ry][j];
             const int e = (tx0 + j + 1 < bw) ? (int)sE[ry][j + 1] : a;
-            v = (int)sH[ry][j + 1] + ((a + e) >> 1);
+            v[2 * t] = a;
+            v[2 * t + 1] = (int)sH[ry][j + 1] + ((a + e) >> 1);
         }
         if (LAST) {
-            v = min(max(v + 128, 0), 255);
-            p.img_out[(size_t)n * p.image_stride + ((size_t)y * p.img_w + x) * p.C + c] = (uint8_t)v;
+#pragma unroll
+            for (int t = 0; t < 16; ++t) v[t] = min(max(v[t] + 128, 0), 255);
+            uint8_t *dst = p.img_out + (size_t)n * p.image_stride + ((size_t)y * p.img_w + x0) * p.C + c;
+            if (vec_ok && x0 + 15 < p.cw) {
+                uint4 q;
+                q.x = (uint32_t)v[0] | ((uint32_t)v[1] << 8) | ((uint32_t)v[2] << 16) | ((uint32_t)v[3] << 24);
+                q.y = (uint32_t)v[4] | ((uint32_t)v[5] << 8) | ((uint32_t)v[6] << 16) | ((uint32_t)v[7] << 24);
+                q.z = (uint32_t)v[8] | ((uint32_t)v[9] << 8) | ((uint32_t)v[10] << 16) | ((uint32_t)v[11] << 24);
+                q.w = (uint32_t)v[12] | ((uint32_t)v[13] << 8) | ((uint32_t)v[14] << 16) | ((uint32_t)v[15] << 24);
+                *reinterpret_cast<uint4 *>(dst) = q;
+            } else {
+#pragma unroll
+                for (int t = 0; t < 16; ++t)
+                    if (x0 + t < p.cw) dst[(size_t)t * p.C] = (uint8_t)v[t];
+            }
         } else {
-            p.ll_out_plane[(size_t)plane * p.ll_out_plane_stride + (size_t)y * p.cw + x] = (int16_t)v;
+            int16_t *dst = p.ll_out_plane + (size_t)plane * p.ll_out_plane_stride + (size_t)y * p.cw + x0;
+            if (vec_ok && x0 + 15 < p.cw) {
+                uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+                d4[0] = make_uint4(pack16(v[0], v[1]), pack16(v[2], v[3]), pack16(v[4], v[5]), pack16(v[6], v[7]));
+                d4[1] = make_uint4(pack16(v[8], v[9]), pack16(v[10], v[11]), pack16(v[12], v[13]), pack16(v[14], v[15]));
+            } else {
+#pragma unroll
+                for (int t = 0; t < 16; ++t)
+                    if (x0 + t < p.cw) dst[t] = (int16_t)v[t];
+            }
         }
     }
 }

@@ -19,16 +19,17 @@ struct MerkleLevelParams {
     unsigned n_trees;
     size_t in_tree_stride, out_tree_stride;  // bytes
     int odd_trees_only_if_nonempty;  // 1: skip odd trees (public fragments) because they are empty (k = 63)
+    uint32_t one;                    // = 1, opaque to the compiler (sha256_compress_rolled_fma)
+    // merkle_tail_kernel only: an optional extra tree of another shape, reduced by CTA number n_trees (DWT: the
+    // private and the public tree finish in one launch)
+    const uint8_t *in2;
+    uint8_t *out2;
+    unsigned n_in2;
 };
 
-__global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid_constant__ MerkleLevelParams p) {
-    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
-    if (gid >= (unsigned long long)p.n_trees * p.n_out) return;
-    const unsigned t = (unsigned)(gid / p.n_out), j = (unsigned)(gid % p.n_out);
-    if (p.odd_trees_only_if_nonempty && (t & 1u)) return;
-    const unsigned lo = j * FANOUT, hi = min(lo + FANOUT, p.n_in), cnt = hi - lo;
-    const uint4 *src = reinterpret_cast<const uint4 *>(p.in + (size_t)t * p.in_tree_stride + (size_t)lo * 32);
-    uint32_t H[8];
+// SHA-256 of `cnt` (1..16) concatenated 32-byte child digests at src (global memory via the read-only path, or shared).
+template <bool GLOBAL, bool LATENCY = false>
+__device__ __forceinline__ void hash_children(const uint4 *src, unsigned cnt, uint32_t (&H)[8], const uint32_t one) {
     sha256_init(H);
     const unsigned pairs = cnt >> 1;
     uint32_t w[16];
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid
         if (i < pairs) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const uint4 v = __ldg(src + 4 * i + q);
+                const uint4 v = GLOBAL ? __ldg(src + 4 * i + q) : src[4 * i + q];
                 w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
             }
         } else {
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid
             if (cnt & 1u) {
 #pragma unroll
                 for (int q = 0; q < 2; ++q) {
-                    const uint4 v = __ldg(src + 4 * i + q);
+                    const uint4 v = GLOBAL ? __ldg(src + 4 * i + q) : src[4 * i + q];
                     w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
                 }
                 w[8] = 0x80000000u;
@@ -56,9 +57,63 @@ __global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid
             }
             w[15] = cnt * 256u;  // message bits = cnt * 32 bytes * 8
         }
-        sha256_compress(H, w);
+        // LATENCY: a lone warp walks the chain, so the shortest dependency path wins (3-input adds, full unroll);
+        // otherwise throughput wins (rolled loop, additions on the FMA pipe).
+        if (LATENCY) sha256_compress(H, w); else sha256_compress_rolled_fma(H, w, one);
     }
+}
+
+__device__ __forceinline__ void digest_to_words(const uint32_t (&H)[8], uint4 &a, uint4 &b) {
+    a = make_uint4(bswap32(H[0]), bswap32(H[1]), bswap32(H[2]), bswap32(H[3]));
+    b = make_uint4(bswap32(H[4]), bswap32(H[5]), bswap32(H[6]), bswap32(H[7]));
+}
+
+__global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid_constant__ MerkleLevelParams p) {
+    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
+    if (gid >= (unsigned long long)p.n_trees * p.n_out) return;
+    const unsigned t = (unsigned)(gid / p.n_out), j = (unsigned)(gid % p.n_out);
+    if (p.odd_trees_only_if_nonempty && (t & 1u)) return;
+    const unsigned lo = j * FANOUT, hi = min(lo + FANOUT, p.n_in), cnt = hi - lo;
+    const uint4 *src = reinterpret_cast<const uint4 *>(p.in + (size_t)t * p.in_tree_stride + (size_t)lo * 32);
+    uint32_t H[8];
+    hash_children<true>(src, cnt, H, p.one);
     store_digest(p.out + (size_t)t * p.out_tree_stride + (size_t)j * 32, H);
+}
+
+// The top of a tree in one launch: one CTA per tree reduces n_in <= 4096 digests to the root (up to three levels of
+// fan-out 16: <= 256 nodes, <= 16 nodes, 1), intermediate levels in shared memory.
+constexpr int TAIL_THREADS = 256;
+constexpr unsigned TAIL_MAX_IN = TAIL_THREADS * FANOUT;
+__global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_constant__ MerkleLevelParams p) {
+    __shared__ uint4 sA[TAIL_THREADS * 2];
+    __shared__ uint4 sB[FANOUT * 2];
+    const unsigned t = blockIdx.x, tid = threadIdx.x;
+    const bool extra = t >= p.n_trees;
+    if (!extra && p.odd_trees_only_if_nonempty && (t & 1u)) return;
+    uint4 *root = reinterpret_cast<uint4 *>(extra ? p.out2 : p.out + (size_t)t * p.out_tree_stride);
+    const uint4 *in = reinterpret_cast<const uint4 *>(extra ? p.in2 : p.in + (size_t)t * p.in_tree_stride);
+    const unsigned n_in = extra ? p.n_in2 : p.n_in;
+    const unsigned n1 = (n_in + FANOUT - 1) / FANOUT;
+    uint32_t H[8];
+    if (tid < n1) {
+        const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n_in) - lo;
+        hash_children<true, true>(in + 2 * (size_t)lo, cnt, H, p.one);
+        digest_to_words(H, sA[2 * tid], sA[2 * tid + 1]);
+    }
+    __syncthreads();
+    if (n1 == 1) { if (tid < 2) root[tid] = sA[tid]; return; }
+    const unsigned n2 = (n1 + FANOUT - 1) / FANOUT;
+    if (tid < n2) {
+        const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n1) - lo;
+        hash_children<false, true>(sA + 2 * lo, cnt, H, p.one);
+        digest_to_words(H, sB[2 * tid], sB[2 * tid + 1]);
+    }
+    __syncthreads();
+    if (n2 == 1) { if (tid < 2) root[tid] = sB[tid]; return; }
+    if (tid == 0) {
+        hash_children<false, true>(sB, n2, H, p.one);
+        digest_to_words(H, root[0], root[1]);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -68,35 +123,42 @@ __global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid
 // the generic byte tail below handles any length).
 // ------------------------------------------------------------------------------------------------------------
 struct StreamLeavesParams {
-    const uint8_t *data;     // stream t at data + t*stream_stride
-    size_t stream_stride;
-    unsigned long long n_bytes;  // per stream
-    unsigned n_leaves;           // per stream
-    unsigned n_streams;
-    uint8_t *out;                // leaf digests [stream][leaf][32] with out_stream_stride bytes between streams
-    size_t out_stream_stride;
+    const uint8_t *data[2];        // the two fragment streams (private, public); hashed in one launch
+    unsigned long long n_bytes[2];
+    unsigned n_leaves[2];
+    uint8_t *out[2];               // leaf digests [leaf][32] per stream
+    uint32_t one;                  // = 1, opaque to the compiler (sha256_compress_rolled_fma)
 };
 
 __global__ void __launch_bounds__(HASH_THREADS) stream_leaves_kernel(const __grid_constant__ StreamLeavesParams p) {
-    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
-    if (gid >= (unsigned long long)p.n_streams * p.n_leaves) return;
-    const unsigned t = (unsigned)(gid / p.n_leaves), j = (unsigned)(gid % p.n_leaves);
+    const unsigned gid = blockIdx.x * HASH_THREADS + threadIdx.x;
+    if (gid >= p.n_leaves[0] + p.n_leaves[1]) return;
+    const int f = gid >= p.n_leaves[0] ? 1 : 0;
+    const unsigned j = f ? gid - p.n_leaves[0] : gid;
     const unsigned long long lo = (unsigned long long)j * DWT_LEAF_BYTES;
-    const unsigned len = (unsigned)min((unsigned long long)DWT_LEAF_BYTES, p.n_bytes - lo);
-    const uint8_t *src = p.data + (size_t)t * p.stream_stride + lo;
+    const unsigned len = (unsigned)min((unsigned long long)DWT_LEAF_BYTES, p.n_bytes[f] - lo);
+    const uint8_t *src = p.data[f] + lo;
     uint32_t H[8];
     sha256_init(H);
     const unsigned full = len >> 6, tail = len & 63u;
     const unsigned nblocks = full + ((tail + 9 <= 64) ? 1u : 2u);
     uint32_t w[16];
+    uint4 nx[4];  // the next 64-byte block is in flight while the current one is compressed
+    if (full > 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) nx[q] = __ldg(reinterpret_cast<const uint4 *>(src) + q);
+    }
 #pragma unroll 1
     for (unsigned i = 0; i < nblocks; ++i) {
         if (i < full) {
-            const uint4 *s4 = reinterpret_cast<const uint4 *>(src + 64 * (size_t)i);
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const uint4 v = __ldg(s4 + q);
-                w[4 * q] = bswap32(v.x); w[4 * q + 1] = bswap32(v.y); w[4 * q + 2] = bswap32(v.z); w[4 * q + 3] = bswap32(v.w);
+                w[4 * q] = bswap32(nx[q].x); w[4 * q + 1] = bswap32(nx[q].y); w[4 * q + 2] = bswap32(nx[q].z); w[4 * q + 3] = bswap32(nx[q].w);
+            }
+            if (i + 1 < full) {
+                const uint4 *s4 = reinterpret_cast<const uint4 *>(src + 64 * (size_t)(i + 1));
+#pragma unroll
+                for (int q = 0; q < 4; ++q) nx[q] = __ldg(s4 + q);
             }
         } else {
             // tail + padding, byte by byte (only the last leaf of a stream ever has a tail)
@@ -115,9 +177,9 @@ __global__ void __launch_bounds__(HASH_THREADS) stream_leaves_kernel(const __gri
             }
             if (i == nblocks - 1) { w[14] = 0u; w[15] = len * 8u; }
         }
-        sha256_compress(H, w);
+        sha256_compress_rolled_fma(H, w, p.one);
     }
-    store_digest(p.out + (size_t)t * p.out_stream_stride + (size_t)j * 32, H);
+    store_digest(p.out[f] + (size_t)j * 32, H);
 }
 
 // ------------------------------------------------------------------------------------------------------------
