@@ -2,7 +2,9 @@
 // Nothing here allocates, synchronises or keeps state across calls (one thread-local last-error slot aside).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/feds.h"
@@ -33,6 +35,13 @@ feds_status cuda_fail(cudaError_t e) {
         if (e__ != cudaSuccess) return cuda_fail(e__);    \
     } while (0)
 #define FEDS_LAUNCH_CHECK() FEDS_CUDA(cudaGetLastError())
+
+// SMs of the current device (the persistent DCT kernels launch one CTA per SM); asked per call, nothing is cached
+int sm_count() {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    return n;
+}
 
 bool dct_dims_ok(int w, int h) { return w > 0 && h > 0 && (w % 8) == 0 && (h % 8) == 0; }
 bool chan_ok(int c) { return c == 1 || c == 3 || c == 4; }
@@ -159,6 +168,7 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
     p.slot_stride = dct_slot_words(k);
     p.one = 1u;
+    p.n_groups = (unsigned)((p.total_leaves + 31) / 32);
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
@@ -176,12 +186,16 @@ feds_status dispatch_cv(const DctParams &p, int c, cudaStream_t stream) {
 
 template <typename Kernel>
 feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream) {
-    const size_t smem = (size_t)(AES_TABLE_WORDS + DCT_THREADS * p.slot_stride) * 4;
-    const unsigned grid = (unsigned)((p.total_leaves + DCT_THREADS - 1) / DCT_THREADS);
+    // persistent: one CTA per SM, its warps stride over the leaf groups. 16 warps unless their slots exceed the SM's
+    // shared memory (k >= 32: the padding slack grows), then 8.
+    int threads = DCT_THREADS;
+    size_t smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4;
+    if (smem > DCT_SMEM_MAX) { threads /= 2; smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4; }
+    const unsigned grid = std::min<unsigned>(p.n_groups, (unsigned)sm_count());
     feds_status s = set_smem(kernel, smem);
     if (s != FEDS_OK) return s;
     if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    kernel<<<grid, DCT_THREADS, smem, stream>>>(p);
+    kernel<<<grid, threads, smem, stream>>>(p);
     if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;

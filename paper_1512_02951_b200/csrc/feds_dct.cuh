@@ -21,8 +21,9 @@ namespace feds {
 
 __device__ const AesTables g_aes = make_aes_tables();
 
-constexpr int DCT_THREADS = 256;
-constexpr int DCT_CTAS_PER_SM = 2;
+constexpr int DCT_THREADS = 512;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
+constexpr int DCT_CTAS_PER_SM = 1;
+constexpr size_t DCT_SMEM_MAX = 227 * 1024;
 constexpr int AES_TABLE_WORDS = 1024;
 constexpr int CA = 16;  // carry area: a SHA-256 block is 16 words, at most 15 (16 - V) words wait between blocks
 
@@ -44,6 +45,7 @@ struct DctParams {
     unsigned long long total_leaves;
     int slot_stride;  // words per lane slot
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
+    unsigned n_groups;  // ceil(total_leaves / 32): one group = the 32 leaves one warp owns at a time
 };
 
 // Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:
@@ -400,7 +402,11 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
     constexpr ZigzagTable ZZ = make_zigzag();
 
     const int k = p.k, P = k + 1, Q = 63 - k;
-    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)blockIdx.x * DCT_THREADS + threadIdx.x);
+    uint32_t *mp = my + CA;      // private words of the current block, indexed by z
+    uint32_t *mq = my + 2 * CA;  // public words of the current block, indexed by z (z >= P)
+#pragma unroll 1
+    for (unsigned grp = (unsigned)warp * gridDim.x + blockIdx.x; grp < p.n_groups; grp += (blockDim.x >> 5) * gridDim.x) {
+    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)grp * 32 + lane);
     const uint8_t *img = p.images + (size_t)L.n * p.image_stride;
     uint32_t *pub_dst = reinterpret_cast<uint32_t *>(p.pub + (size_t)L.n * p.pub_stride) + (size_t)L.b0 * Q;
     uint32_t *priv_dst = reinterpret_cast<uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
@@ -416,8 +422,6 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
     Keystream K;
     K.blk = ~0ull;
     const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
-    uint32_t *mp = my + CA;      // private words of the current block, indexed by z
-    uint32_t *mq = my + 2 * CA;  // public words of the current block, indexed by z (z >= P)
 
 #pragma unroll 1
     for (int s = 0; s <= G_BLOCKS; ++s) {
@@ -475,6 +479,8 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
         store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, oth.H);
         if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
     }
+    if (V == 1) __syncwarp();  // the next group's first copy-out reads every lane's slot
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -491,7 +497,11 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
     constexpr ZigzagTable ZZ = make_zigzag();
 
     const int k = p.k, P = k + 1, Q = 63 - k;
-    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)blockIdx.x * DCT_THREADS + threadIdx.x);
+    uint32_t *mp = my + CA;
+    uint32_t *mq = my + 2 * CA;
+#pragma unroll 1
+    for (unsigned grp = (unsigned)warp * gridDim.x + blockIdx.x; grp < p.n_groups; grp += (blockDim.x >> 5) * gridDim.x) {
+    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)grp * 32 + lane);
     uint8_t *img = p.images_out + (size_t)L.n * p.image_stride;
     const uint32_t *pub_src = reinterpret_cast<const uint32_t *>(p.pub + (size_t)L.n * p.pub_stride) + (size_t)L.b0 * Q;
     const uint32_t *priv_src = reinterpret_cast<const uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
@@ -505,8 +515,6 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
     Keystream K;
     K.blk = ~0ull;
     const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
-    uint32_t *mp = my + CA;
-    uint32_t *mq = my + 2 * CA;
 
 #pragma unroll 1
     for (int s = 0; s <= G_BLOCKS; ++s) {
@@ -575,6 +583,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
         const size_t nl = p.leaves_per_image;
         store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, oth.H);
         if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
+    }
     }
 }
 
