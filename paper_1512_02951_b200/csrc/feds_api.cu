@@ -185,12 +185,12 @@ feds_status dispatch_cv(const DctParams &p, int c, cudaStream_t stream) {
 }
 
 template <typename Kernel>
-feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream) {
+feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream, int max_threads = DCT_THREADS) {
     // persistent: one CTA per SM, its warps stride over the leaf groups. 16 warps unless their slots exceed the SM's
     // shared memory (k >= 32: the padding slack grows), then 8.
-    int threads = DCT_THREADS;
+    int threads = max_threads;
     size_t smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4;
-    if (smem > DCT_SMEM_MAX) { threads /= 2; smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4; }
+    if (smem > DCT_SMEM_MAX) { threads = 256; smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4; }
     const unsigned grid = std::min<unsigned>(p.n_groups, (unsigned)sm_count());
     feds_status s = set_smem(kernel, smem);
     if (s != FEDS_OK) return s;
@@ -203,8 +203,8 @@ feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream) {
 
 template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, true>, p, s); } };
 template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, false>, p, s); } };
-template <int C, int V> struct DefragVerify { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, true>, p, s); } };
-template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, false>, p, s); } };
+template <int C, int V> struct DefragVerify { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, true>, p, s, DEFRAG_THREADS); } };
+template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, false>, p, s, DEFRAG_THREADS); } };
 
 template <bool DIGEST>
 feds_status launch_fragment(const DctParams &p, int c, cudaStream_t stream) {

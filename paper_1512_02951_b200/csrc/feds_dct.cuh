@@ -21,9 +21,16 @@ namespace feds {
 
 __device__ const AesTables g_aes = make_aes_tables();
 
-constexpr int DCT_THREADS = 512;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
+#ifndef FEDS_FRAG_THREADS
+#define FEDS_FRAG_THREADS 512
+#endif
+constexpr int DCT_THREADS = FEDS_FRAG_THREADS;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
 constexpr int DCT_CTAS_PER_SM = 1;
 constexpr size_t DCT_SMEM_MAX = 227 * 1024;
+#ifndef FEDS_DEFRAG_THREADS
+#define FEDS_DEFRAG_THREADS 384
+#endif
+constexpr int DEFRAG_THREADS = FEDS_DEFRAG_THREADS;
 constexpr int AES_TABLE_WORDS = 1024;
 constexpr int CA = 16;  // carry area: a SHA-256 block is 16 words, at most 15 (16 - V) words wait between blocks
 
@@ -56,10 +63,12 @@ struct DctParams {
 __host__ __device__ inline int dct_vec_width(int k) { return ((k + 1) % 4 == 0) ? 4 : ((k + 1) % 2 == 0) ? 2 : 1; }
 __host__ __device__ inline int dct_slot_words(int k) {
     const int Q = 63 - k, V = dct_vec_width(k);
-    int wds = 2 * CA + 64 + (Q < 32 ? 32 - Q : 0);
+    int wds = 2 * CA + 64 + (Q < 32 ? 32 - Q : 0) + 8;  // + 8: the waiting stream's chaining value (dct_stash_offset)
     while (wds % (2 * V) != V) ++wds;
     return wds;
 }
+
+__host__ __device__ inline int dct_stash_offset(int k) { const int Q = 63 - k; return 2 * CA + 64 + (Q < 32 ? 32 - Q : 0); }
 
 template <int V> struct VecT;
 template <> struct VecT<1> { using type = uint32_t; };
@@ -233,6 +242,12 @@ __device__ __forceinline__ void load_nonce(const DctParams &p, int n, uint32_t (
 
 // One SHA-256 stream living in a lane's slot: `carry` words wait at [base+16-carry, base+16), `fresh` new words
 // were just written at [base+16, base+16+fresh). Compress every full 16-word block, slide the rest down.
+struct ShaMeta {
+    int base;
+    int carry;
+    int fresh;
+    unsigned total_words;
+};
 struct ShaStream {
     uint32_t H[8];
     int base;
@@ -241,14 +256,47 @@ struct ShaStream {
     unsigned total_words;  // message length of the whole leaf in 32-bit words (0: stream unused)
 };
 
-__device__ __forceinline__ void swap_streams(ShaStream &a, ShaStream &b) {
+// Only the stream being absorbed keeps its chaining value in registers; the other one's waits in the lane's slot at
+// word offset `hoff` (8 words). 16 fewer live registers across the compression loop than a register swap.
+template <int V>
+__device__ __forceinline__ void swap_streams(uint32_t *my, int hoff, ShaStream &a, ShaMeta &b) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { const uint32_t t = a.H[i]; a.H[i] = b.H[i]; b.H[i] = t; }
+    for (int i = 0; i < 8; i += V) {
+        uint32_t t[V], u[V];
+        vec_load<V>(my + hoff + i, t);
+#pragma unroll
+        for (int j = 0; j < V; ++j) u[j] = a.H[i + j];
+        vec_store<V>(my + hoff + i, u);
+#pragma unroll
+        for (int j = 0; j < V; ++j) a.H[i + j] = t[j];
+    }
     int t;
     t = a.base; a.base = b.base; b.base = t;
     t = a.carry; a.carry = b.carry; b.carry = t;
     t = a.fresh; a.fresh = b.fresh; b.fresh = t;
     const unsigned u = a.total_words; a.total_words = b.total_words; b.total_words = u;
+}
+template <int V>
+__device__ __forceinline__ void stash_init(uint32_t *my, int hoff) {
+    uint32_t H[8];
+    sha256_init(H);
+#pragma unroll
+    for (int i = 0; i < 8; i += V) {
+        uint32_t u[V];
+#pragma unroll
+        for (int j = 0; j < V; ++j) u[j] = H[i + j];
+        vec_store<V>(my + hoff + i, u);
+    }
+}
+template <int V>
+__device__ __forceinline__ void stash_read(const uint32_t *my, int hoff, uint32_t (&H)[8]) {
+#pragma unroll
+    for (int i = 0; i < 8; i += V) {
+        uint32_t t[V];
+        vec_load<V>(my + hoff + i, t);
+#pragma unroll
+        for (int j = 0; j < V; ++j) H[i + j] = t[j];
+    }
 }
 
 // Append the FIPS 180-4 5.1.1 padding for a message of `total_words` 32-bit words after the carried words.
@@ -415,8 +463,11 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
 
     // cur = public stream, oth = private stream (swapped twice per phase). The public stream goes first so that in the
     // final phase the private stream's padding may spill into the (then finished) public region.
-    ShaStream cur, oth;
-    sha256_init(cur.H); sha256_init(oth.H);
+    ShaStream cur;
+    ShaMeta oth;
+    const int hoff = dct_stash_offset(k);
+    sha256_init(cur.H);
+    if (DIGEST) stash_init<V>(my, hoff);
     cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
     oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
     Keystream K;
@@ -470,14 +521,15 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
                 absorb<V>(my, cur, p.one);
-                swap_streams(cur, oth);
+                swap_streams<V>(my, hoff, cur, oth);
             }
         }
     }
     if (DIGEST && L.valid) {
         const size_t nl = p.leaves_per_image;
-        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, oth.H);
         if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
+        stash_read<V>(my, hoff, cur.H);  // after an even number of swaps the private stream is the stashed one
+        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
     }
     if (V == 1) __syncwarp();  // the next group's first copy-out reads every lane's slot
     }
@@ -487,7 +539,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
 // defragment: steps 6-8 (+ recomputation of the leaf digests of the fragments as received when VERIFY)
 // ------------------------------------------------------------------------------------------------------------
 template <int C, int V, bool VERIFY>
-__global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_kernel(const __grid_constant__ DctParams p) {
+__global__ void __launch_bounds__(DEFRAG_THREADS, DCT_CTAS_PER_SM) defragment_dct_kernel(const __grid_constant__ DctParams p) {
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
     load_aes_tables(sT);
@@ -508,8 +560,11 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
     uint32_t nonce[4];
     load_nonce(p, L.n, nonce);
 
-    ShaStream cur, oth;
-    sha256_init(cur.H); sha256_init(oth.H);
+    ShaStream cur;
+    ShaMeta oth;
+    const int hoff = dct_stash_offset(k);
+    sha256_init(cur.H);
+    if (VERIFY) stash_init<V>(my, hoff);
     cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
     oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
     Keystream K;
@@ -550,7 +605,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
             for (int it = 0; it < 2; ++it) {
                 if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
                 absorb<V>(my, cur, p.one);  // hashes the bytes as received; leaves [base+16, ..) of the current block intact
-                swap_streams(cur, oth);
+                swap_streams<V>(my, hoff, cur, oth);
             }
         }
         if (s < G_BLOCKS) {
@@ -581,8 +636,9 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) defragment_dct_k
     }
     if (VERIFY && L.valid) {
         const size_t nl = p.leaves_per_image;
-        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, oth.H);
         if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
+        stash_read<V>(my, hoff, cur.H);  // after an even number of swaps the private stream is the stashed one
+        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
     }
     }
 }
