@@ -150,6 +150,29 @@ feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_
                                      size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags);
 
 /*
+ * Stream primitives: the two cryptographic steps of the path on a plain byte stream in device memory.
+ *
+ * feds_aes128_ctr — step 4 alone: d_out[i] = d_in[i] XOR keystream[i] over n_bytes bytes, counter block of the j-th
+ * 16-byte block = (nonce + j) mod 2^128 big-endian (SP 800-38A 6.5, A6); the keystream of a partial last block
+ * is truncated. d_out == d_in (in place) is allowed, partial overlap is not. This is also the report's comparison
+ * baseline "AES over the whole image" when given the image bytes.
+ * key, nonce: HOST pointers. n_bytes == 0 is a no-op.
+ *
+ * feds_sha256_merkle — step 5 alone on a stream: leaf j = SHA-256(bytes [2048 j, min(2048 (j+1), n))), upper levels with
+ * fan-out 16; a one-leaf stream's root is its leaf digest, an empty stream's root is SHA-256("").
+ * d_root: 32 bytes, device. Workspace: feds_sha256_merkle_workspace_bytes(n_bytes) (leaf and inner digests); may be
+ * NULL when the stream has at most one leaf.
+ *
+ * Errors as for the other entry points: NULL_POINTER, MISALIGNED (16-byte alignment of every device pointer),
+ * WORKSPACE_TOO_SMALL, BAD_PARAM (more than 2^32 - 1 leaves), CUDA. Nothing is enqueued when an error is returned.
+ */
+feds_status feds_aes128_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16],
+                            const uint8_t nonce[16], feds_stream_t stream);
+size_t feds_sha256_merkle_workspace_bytes(size_t n_bytes);
+feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d_root, void *d_workspace,
+                               size_t workspace_bytes, feds_stream_t stream);
+
+/*
  * Profiling hook (not part of the data path; thread-local): while set, every DCT fragment/defragment call made on this
  * thread records ev_start immediately before and ev_stop immediately after its fused tile kernel, on the call's stream.
  * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.

@@ -26,6 +26,7 @@ SYMBOLS = [
     "feds_fragment_dct_batch", "feds_defragment_dct_batch",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
+    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
 ]
 
@@ -62,6 +63,10 @@ def _load():
     lib.feds_defragment_dct_host_scratch_bytes.restype = sz
     lib.feds_defragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_defragment_dct_host.argtypes = [vp, vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
+    lib.feds_aes128_ctr.argtypes = [vp, vp, sz, u8p, u8p, vp]
+    lib.feds_sha256_merkle_workspace_bytes.restype = sz
+    lib.feds_sha256_merkle_workspace_bytes.argtypes = [sz]
+    lib.feds_sha256_merkle.argtypes = [vp, sz, vp, vp, sz, vp]
     lib.feds_profile_events.argtypes = [vp, vp]
     lib.feds_profile_events.restype = None
     lib.feds_debug_sha256_host.argtypes = [u8p, sz, vp]
@@ -69,7 +74,8 @@ def _load():
     lib.feds_debug_dct8x8_host.argtypes = [vp, vp, i]
     lib.feds_debug_zigzag_host.argtypes = [vp]
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
-                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host"]:
+                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host",
+                 "feds_aes128_ctr", "feds_sha256_merkle"]:
         getattr(lib, name).restype = i
     return lib
 
@@ -173,6 +179,26 @@ def defragment_dwt(priv, pub, w, h, c, levels, key, nonce, expected=None, stream
     _check(lib.feds_defragment_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, bytes(key), bytes(nonce), _ptr(expected), _ptr(out),
                                    _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dwt")
     return out, flags
+
+
+def aes128_ctr(data, key, nonce, out=None, stream=None):
+    """feds_aes128_ctr on a uint8 device tensor; out=None allocates, out=data works in place."""
+    data = data.contiguous().view(-1)
+    if out is None:
+        out = torch.empty_like(data)
+    _check(lib.feds_aes128_ctr(_ptr(data), _ptr(out), data.numel(), bytes(key), bytes(nonce), _stream(stream)), "feds_aes128_ctr")
+    return out
+
+
+def sha256_merkle(data, stream=None, workspace=None):
+    """feds_sha256_merkle: 32-byte Merkle root (2048-byte leaves, fan-out 16) of a uint8 device tensor."""
+    data = data.contiguous().view(-1)
+    root = _u8(32, data.device)
+    need = lib.feds_sha256_merkle_workspace_bytes(data.numel())
+    ws = workspace if workspace is not None else _u8(max(need, 16), data.device)
+    _check(lib.feds_sha256_merkle(_ptr(data) if data.numel() else None, data.numel(), _ptr(root), _ptr(ws), ws.numel(), _stream(stream)),
+           "feds_sha256_merkle")
+    return root
 
 
 class DctBatch:

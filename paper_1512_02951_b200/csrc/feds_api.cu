@@ -337,6 +337,29 @@ size_t dwt_level_off_elems(int w, int h, int L, int l) {  // elements before lev
     return off;
 }
 
+// AES-128-CTR of a byte stream: the conflict-free 128 KB table layout pays once the stream is a few MB long
+feds_status launch_aes_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16], const uint8_t nonce[16],
+                           cudaStream_t stream) {
+    if (n_bytes == 0) return FEDS_OK;
+    CtrParams cp{};
+    cp.in = d_in; cp.out = d_out; cp.n_bytes = n_bytes;
+    nonce_to_be(nonce, cp.nonce_be);
+    aes128_expand_key_host(key, cp.rk, h_aes);
+    const unsigned long long nblk = (n_bytes + 15) / 16;
+    const unsigned sms = (unsigned)sm_count();
+    if (n_bytes >= ((size_t)4 << 20)) {
+        const size_t smem = (size_t)AES_TABLE_WORDS * 32 * 4;
+        feds_status st = set_smem(aes_ctr_stream_kernel<32>, smem);
+        if (st != FEDS_OK) return st;
+        aes_ctr_stream_kernel<32><<<sms, AES_THREADS, smem, stream>>>(cp);
+    } else {
+        const unsigned want = (unsigned)((nblk + AES_THREADS - 1) / AES_THREADS);
+        aes_ctr_stream_kernel<1><<<std::min(want, 2 * sms), AES_THREADS, (size_t)AES_TABLE_WORDS * 4, stream>>>(cp);
+    }
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
 feds_status dwt_digests(const uint8_t *d_private, const uint8_t *d_public, const DwtPlan &pl, uint8_t *tree_ws, uint8_t *roots,
                         cudaStream_t stream) {
     const unsigned nls[2] = {pl.priv_nl, pl.pub_nl};
@@ -482,13 +505,8 @@ feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int l
         else dwt_fwd_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
         FEDS_LAUNCH_CHECK();
     }
-    CtrParams cp{};
-    cp.data = d_private; cp.stream_stride = 0; cp.n_bytes = pl.priv_b; cp.n_streams = 1; cp.d_nonces = nullptr;
-    nonce_to_be(nonce, cp.nonce_be);
-    aes128_expand_key_host(key, cp.rk, h_aes);
-    const unsigned long long nblk = (pl.priv_b + 15) / 16;
-    aes_ctr_kernel<<<(unsigned)((nblk + HASH_THREADS - 1) / HASH_THREADS), HASH_THREADS, 0, stream>>>(cp);
-    FEDS_LAUNCH_CHECK();
+    const feds_status st = launch_aes_ctr(d_private, d_private, pl.priv_b, key, nonce, stream);
+    if (st != FEDS_OK) return st;
     return dwt_digests(d_private, d_public, pl, ws + pl.planes_bytes, d_digests, stream);
 }
 
@@ -515,16 +533,12 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
         compare_digests_kernel<<<1, 32, 0, stream>>>(roots, d_expected_digests, d_verify_flags, 1);
         FEDS_LAUNCH_CHECK();
     }
-    // decrypt a copy of LL_L into the level-L plane block
+    // decrypt LL_L into the level-L plane block (the received fragment stays untouched)
     uint8_t *lldec = ws + pl.plane_off[L];
-    FEDS_CUDA(cudaMemcpyAsync(lldec, d_private, pl.priv_b, cudaMemcpyDeviceToDevice, stream));
-    CtrParams cp{};
-    cp.data = lldec; cp.stream_stride = 0; cp.n_bytes = pl.priv_b; cp.n_streams = 1; cp.d_nonces = nullptr;
-    nonce_to_be(nonce, cp.nonce_be);
-    aes128_expand_key_host(key, cp.rk, h_aes);
-    const unsigned long long nblk = (pl.priv_b + 15) / 16;
-    aes_ctr_kernel<<<(unsigned)((nblk + HASH_THREADS - 1) / HASH_THREADS), HASH_THREADS, 0, stream>>>(cp);
-    FEDS_LAUNCH_CHECK();
+    {
+        const feds_status st = launch_aes_ctr(d_private, lldec, pl.priv_b, key, nonce, stream);
+        if (st != FEDS_OK) return st;
+    }
 
     for (int l = L; l >= 1; --l) {
         DwtLevelParams p{};
@@ -544,6 +558,46 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
         else dwt_inv_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
         FEDS_LAUNCH_CHECK();
     }
+    return FEDS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ stream primitives
+feds_status feds_aes128_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16], const uint8_t nonce[16],
+                            feds_stream_t stream) {
+    if (!key || !nonce || (n_bytes && (!d_in || !d_out))) return FEDS_ERR_NULL_POINTER;
+    if (misaligned(d_in) || misaligned(d_out)) return FEDS_ERR_MISALIGNED;
+    return launch_aes_ctr(d_in, d_out, n_bytes, key, nonce, stream);
+}
+
+size_t feds_sha256_merkle_workspace_bytes(size_t n_bytes) {
+    const size_t nl = (n_bytes + DWT_LEAF_BYTES - 1) / DWT_LEAF_BYTES;
+    if (nl > 0xffffffffull) return 0;
+    return round_up(tree_bytes((unsigned)nl) + 32, 256);
+}
+
+feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d_root, void *d_workspace, size_t workspace_bytes,
+                               feds_stream_t stream) {
+    if (!d_root || (n_bytes && !d_data)) return FEDS_ERR_NULL_POINTER;
+    if (misaligned(d_data) || misaligned(d_root) || misaligned(d_workspace)) return FEDS_ERR_MISALIGNED;
+    const size_t nl64 = (n_bytes + DWT_LEAF_BYTES - 1) / DWT_LEAF_BYTES;
+    if (nl64 > 0xffffffffull) return FEDS_ERR_BAD_PARAM;
+    const unsigned nl = (unsigned)nl64;
+    if (nl > 1 && (!d_workspace || workspace_bytes < feds_sha256_merkle_workspace_bytes(n_bytes))) return d_workspace ? FEDS_ERR_WORKSPACE_TOO_SMALL : FEDS_ERR_NULL_POINTER;
+    if (nl == 0) {  // SHA-256(""): the kernel writes it at digests + 32
+        uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+        (void)ws;
+        write_empty_root_kernel<<<1, 32, 0, stream>>>(d_root);
+        FEDS_LAUNCH_CHECK();
+        return FEDS_OK;
+    }
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    StreamLeavesParams sp{};
+    sp.data[0] = d_data; sp.n_bytes[0] = n_bytes; sp.n_leaves[0] = nl;
+    sp.out[0] = nl > 1 ? ws : d_root;
+    sp.one = 1u;
+    stream_leaves_kernel<<<(nl + HASH_THREADS - 1) / HASH_THREADS, HASH_THREADS, 0, stream>>>(sp);
+    FEDS_LAUNCH_CHECK();
+    if (nl > 1) return run_tree(ws, nl, 1, ws + (size_t)nl * 32, d_root, 32, 0, stream);
     return FEDS_OK;
 }
 

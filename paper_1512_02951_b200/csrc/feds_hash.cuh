@@ -183,44 +183,55 @@ __global__ void __launch_bounds__(HASH_THREADS) stream_leaves_kernel(const __gri
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// AES-128-CTR over a byte stream, in place: one thread per 16-byte block (A6). n_bytes per stream.
+// AES-128-CTR over a byte stream (A6): out = in XOR keystream, in place when out == in. Persistent CTAs,
+// threads stride over the 16-byte blocks with 128-bit accesses. REPL = copies of each round-table entry in shared
+// memory: 1 (4 KB; random lookups collide in the 32 banks, ~3.4 wavefronts each) for short streams, 32 (128 KB; lane l
+// reads copy l, which lies in bank l: every lookup is one wavefront) for long ones, where the table fill is amortised.
 // ------------------------------------------------------------------------------------------------------------
 struct CtrParams {
-    uint8_t *data;
-    size_t stream_stride;
+    const uint8_t *in;
+    uint8_t *out;
     unsigned long long n_bytes;
-    unsigned n_streams;
-    const uint8_t *d_nonces;
     uint32_t nonce_be[4];
     uint32_t rk[44];
 };
+constexpr int AES_THREADS = 512;
 
-__global__ void __launch_bounds__(HASH_THREADS) aes_ctr_kernel(const __grid_constant__ CtrParams p) {
-    __shared__ uint32_t sT[AES_TABLE_WORDS];
-    load_aes_tables(sT);
-    const unsigned long long nblk = (p.n_bytes + 15) >> 4;
-    const unsigned long long gid = (unsigned long long)blockIdx.x * HASH_THREADS + threadIdx.x;
-    if (gid >= nblk * p.n_streams) return;
-    const unsigned t = (unsigned)(gid / nblk);
-    const unsigned long long i = gid % nblk;
-    uint32_t nonce[4];
-    if (p.d_nonces) {
-        const uint4 q = __ldg(reinterpret_cast<const uint4 *>(p.d_nonces) + t);
-        nonce[0] = bswap32(q.x); nonce[1] = bswap32(q.y); nonce[2] = bswap32(q.z); nonce[3] = bswap32(q.w);
-    } else {
-        nonce[0] = p.nonce_be[0]; nonce[1] = p.nonce_be[1]; nonce[2] = p.nonce_be[2]; nonce[3] = p.nonce_be[3];
+template <int REPL>
+struct ReplTable {
+    const uint32_t *b;
+    __device__ __forceinline__ uint32_t operator[](unsigned i) const { return b[i * REPL]; }
+};
+
+template <int REPL>
+__global__ void __launch_bounds__(AES_THREADS) aes_ctr_stream_kernel(const __grid_constant__ CtrParams p) {
+    extern __shared__ __align__(16) uint32_t sTab[];
+    {
+        const uint32_t *src = &g_aes.T[0][0];
+        for (int i = threadIdx.x; i < AES_TABLE_WORDS * REPL; i += AES_THREADS) sTab[i] = src[i / REPL];
+        __syncthreads();
     }
-    uint32_t ks[4];
-    ctr_block(nonce, i, ks);
-    aes128_encrypt(sT, p.rk, ks);
-    uint8_t *dst = p.data + (size_t)t * p.stream_stride + 16 * i;
-    if (16 * i + 16 <= p.n_bytes) {
-        uint4 v = *reinterpret_cast<uint4 *>(dst);
+    ReplTable<REPL> T;
+    T.b = sTab + (REPL > 1 ? (threadIdx.x & (REPL - 1)) : 0);
+    const unsigned long long nfull = p.n_bytes >> 4;
+    const unsigned long long stride = (unsigned long long)gridDim.x * AES_THREADS;
+    const uint32_t nonce[4] = {p.nonce_be[0], p.nonce_be[1], p.nonce_be[2], p.nonce_be[3]};
+    const uint4 *in4 = reinterpret_cast<const uint4 *>(p.in);
+    uint4 *out4 = reinterpret_cast<uint4 *>(p.out);
+    for (unsigned long long i = (unsigned long long)blockIdx.x * AES_THREADS + threadIdx.x; i < nfull; i += stride) {
+        uint4 v = __ldg(in4 + i);
+        uint32_t ks[4];
+        ctr_block(nonce, i, ks);
+        aes128_encrypt(T, p.rk, ks);
         v.x ^= ks[0]; v.y ^= ks[1]; v.z ^= ks[2]; v.w ^= ks[3];
-        *reinterpret_cast<uint4 *>(dst) = v;
-    } else {
-        const unsigned rem = (unsigned)(p.n_bytes - 16 * i);
-        for (unsigned b = 0; b < rem; ++b) dst[b] ^= (uint8_t)(ks[b >> 2] >> (8 * (b & 3)));
+        out4[i] = v;
+    }
+    const unsigned rem = (unsigned)(p.n_bytes & 15u);
+    if (rem && blockIdx.x == 0 && threadIdx.x == 0) {  // keystream of the partial last block is truncated
+        uint32_t ks[4];
+        ctr_block(nonce, nfull, ks);
+        aes128_encrypt(T, p.rk, ks);
+        for (unsigned b = 0; b < rem; ++b) p.out[16 * nfull + b] = p.in[16 * nfull + b] ^ (uint8_t)(ks[b >> 2] >> (8 * (b & 3)));
     }
 }
 
@@ -246,6 +257,18 @@ __global__ void write_empty_public_root_kernel(uint8_t *digests, int n_images) {
     w[0] = 0x80000000u;
     sha256_compress(H, w);
     store_digest(digests + 64 * (size_t)n + 32, H);
+}
+
+// SHA-256("") as the root of an empty stream
+__global__ void write_empty_root_kernel(uint8_t *root) {
+    if (threadIdx.x != 0) return;
+    uint32_t H[8], w[16];
+    sha256_init(H);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) w[i] = 0u;
+    w[0] = 0x80000000u;
+    sha256_compress(H, w);
+    store_digest(root, H);
 }
 
 }  // namespace feds
