@@ -11,6 +11,7 @@
 #include "feds_dct.cuh"
 #include "feds_device.cuh"
 #include "feds_dwt.cuh"
+#include "feds_dwt_fast.cuh"
 #include "feds_hash.cuh"
 
 using namespace feds;
@@ -337,6 +338,23 @@ size_t dwt_level_off_elems(int w, int h, int L, int l) {  // elements before lev
     return off;
 }
 
+// Which level kernel: the register-streaming ones (feds_dwt_fast.cuh) need whole per-thread runs and aligned vector
+// accesses; returns the pixels per thread (16: planar int16 or gray uint8; 8: interleaved RGB uint8) or 0 = tiled kernel.
+int dwt_fast_px(const DwtLevelParams &p, bool u8, int c_img) {
+    if (getenv("FEDS_DWT_TILED")) return 0;
+    const int px = u8 ? (c_img == 1 ? 16 : c_img == 3 ? 8 : 0) : 16;
+    if (px == 0 || p.cw % px != 0 || (p.ch & 1)) return 0;
+    const size_t a = (size_t)px / 2;  // subband elements per thread and row: every offset must be a multiple of it
+    if (p.level_off % a || (c_img > 1 && (p.pub_chan_stride % a || p.ll_band_chan_stride % a))) return 0;
+    if ((reinterpret_cast<uintptr_t>(p.ll_band) | reinterpret_cast<uintptr_t>(p.pub)) & 15u) return 0;
+    if (u8) { if (p.img_w % (c_img == 1 ? 16 : 8)) return 0; }
+    return px;
+}
+dim3 dwt_fast_grid(const DwtLevelParams &p, int px, int planes) {
+    const int runs = p.cw / px, bh = p.ch >> 1;
+    return dim3((runs + DWTF_LANES_OUT - 1) / DWTF_LANES_OUT, (bh + DWTF_WARPS * DWTF_ROWS - 1) / (DWTF_WARPS * DWTF_ROWS), planes);
+}
+
 // AES-128-CTR of a byte stream: the conflict-free 128 KB table layout pays once the stream is a few MB long
 feds_status launch_aes_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16], const uint8_t nonce[16],
                            cudaStream_t stream) {
@@ -500,9 +518,15 @@ feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int l
         p.pub_image_stride = pl.pub_b / 2;
         p.pub_chan_stride = pl.pub_b / 2 / c;
         p.level_off = dwt_level_off_elems(w, h, L, l);
-        const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
-        if (l == 1) dwt_fwd_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
-        else dwt_fwd_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
+        const int px = dwt_fast_px(p, l == 1, c);
+        if (px && l == 1 && c == 1) dwt_fwd_fast_kernel<1, 16, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px && l == 1) dwt_fwd_fast_kernel<3, 8, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px) dwt_fwd_fast_kernel<1, 16, false><<<dwt_fast_grid(p, px, c), DWTF_WARPS * 32, 0, stream>>>(p);
+        else {
+            const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
+            if (l == 1) dwt_fwd_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
+            else dwt_fwd_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
+        }
         FEDS_LAUNCH_CHECK();
     }
     const feds_status st = launch_aes_ctr(d_private, d_private, pl.priv_b, key, nonce, stream);
@@ -553,9 +577,15 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
         p.level_off = dwt_level_off_elems(w, h, L, l);
         p.img_out = d_image_out;
         if (l > 1) { p.ll_out_plane = reinterpret_cast<int16_t *>(ws + pl.plane_off[l - 1]); p.ll_out_plane_stride = (size_t)p.cw * p.ch; }
-        const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
-        if (l == 1) dwt_inv_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
-        else dwt_inv_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
+        const int px = dwt_fast_px(p, l == 1, c);
+        if (px && l == 1 && c == 1) dwt_inv_fast_kernel<1, 16, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px && l == 1) dwt_inv_fast_kernel<3, 8, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px) dwt_inv_fast_kernel<1, 16, false><<<dwt_fast_grid(p, px, c), DWTF_WARPS * 32, 0, stream>>>(p);
+        else {
+            const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
+            if (l == 1) dwt_inv_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
+            else dwt_inv_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
+        }
         FEDS_LAUNCH_CHECK();
     }
     return FEDS_OK;

@@ -61,3 +61,24 @@ def test_dwt_verify_flags(orc, b):
 def test_config4_full_size(orc, b):
     """8192x8192 grayscale, 3 levels (BASELINE config 4): bit-exact on everything."""
     run_case(orc, b, synth.image(8192, 8192, 1, seed=4), 3, seed=4)
+
+
+@pytest.mark.parametrize("w,h,c,L", [(1024, 320, 3, 4), (2048, 64, 1, 1), (7696, 96, 1, 2), (496, 80, 3, 1)])
+def test_streaming_and_tiled_level_kernels_agree(orc, b, w, h, c, L, monkeypatch):
+    """The register-streaming level kernels (several column strips, halo lanes, row tiles) and the tiled shared-memory
+    kernels they replace on aligned sizes compute identical fragments; the oracle decides which is right."""
+    img = synth.image(w, h, c, seed=w + L)
+    key, nonce = synth.key_nonce(w)
+    d_img = torch.from_numpy(img).cuda()
+    fast = b.fragment_dwt(d_img, L, key, nonce)
+    monkeypatch.setenv("FEDS_DWT_TILED", "1")
+    tiled = b.fragment_dwt(d_img, L, key, nonce)
+    rec_tiled, _ = b.defragment_dwt(fast[0], fast[1], w, h, c, L, key, nonce)
+    monkeypatch.delenv("FEDS_DWT_TILED")
+    rec_fast, _ = b.defragment_dwt(tiled[0], tiled[1], w, h, c, L, key, nonce)
+    torch.cuda.synchronize()
+    for x, y in zip(fast, tiled):
+        assert torch.equal(x, y)
+    op, oq, odg = orc.fragment_dwt(img, L, key, nonce)
+    assert (fast[0].cpu().numpy() == op).all() and (fast[1].cpu().numpy() == oq).all() and fast[2].cpu().numpy().tobytes() == odg
+    assert torch.equal(rec_tiled, d_img) and torch.equal(rec_fast, d_img)
