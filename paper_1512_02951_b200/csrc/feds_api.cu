@@ -391,7 +391,7 @@ feds_status dwt_digests(const uint8_t *d_private, const uint8_t *d_public, const
         sp.out[f] = nls[f] > 1 ? ws[f] : roots + 32 * f;  // a one-leaf fragment's root is its leaf digest
     }
     const unsigned total = nls[0] + nls[1];
-    stream_leaves_kernel<<<(total + HASH_THREADS - 1) / HASH_THREADS, HASH_THREADS, 0, stream>>>(sp);
+    stream_leaves_kernel<<<(total + LEAF_THREADS - 1) / LEAF_THREADS, LEAF_THREADS, 0, stream>>>(sp);
     FEDS_LAUNCH_CHECK();
     return run_two_trees(ws[0], nls[0], ws[0] + (size_t)nls[0] * 32, roots, ws[1], nls[1], ws[1] + (size_t)nls[1] * 32, roots + 32, stream);
 }
@@ -625,7 +625,7 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
     sp.data[0] = d_data; sp.n_bytes[0] = n_bytes; sp.n_leaves[0] = nl;
     sp.out[0] = nl > 1 ? ws : d_root;
     sp.one = 1u;
-    stream_leaves_kernel<<<(nl + HASH_THREADS - 1) / HASH_THREADS, HASH_THREADS, 0, stream>>>(sp);
+    stream_leaves_kernel<<<(nl + LEAF_THREADS - 1) / LEAF_THREADS, LEAF_THREADS, 0, stream>>>(sp);
     FEDS_LAUNCH_CHECK();
     if (nl > 1) return run_tree(ws, nl, 1, ws + (size_t)nl * 32, d_root, 32, 0, stream);
     return FEDS_OK;

@@ -91,28 +91,27 @@ __global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_
     const bool extra = t >= p.n_trees;
     if (!extra && p.odd_trees_only_if_nonempty && (t & 1u)) return;
     uint4 *root = reinterpret_cast<uint4 *>(extra ? p.out2 : p.out + (size_t)t * p.out_tree_stride);
-    const uint4 *in = reinterpret_cast<const uint4 *>(extra ? p.in2 : p.in + (size_t)t * p.in_tree_stride);
-    const unsigned n_in = extra ? p.n_in2 : p.n_in;
-    const unsigned n1 = (n_in + FANOUT - 1) / FANOUT;
-    uint32_t H[8];
-    if (tid < n1) {
-        const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n_in) - lo;
-        hash_children<true, true>(in + 2 * (size_t)lo, cnt, H, p.one);
-        digest_to_words(H, sA[2 * tid], sA[2 * tid + 1]);
-    }
-    __syncthreads();
-    if (n1 == 1) { if (tid < 2) root[tid] = sA[tid]; return; }
-    const unsigned n2 = (n1 + FANOUT - 1) / FANOUT;
-    if (tid < n2) {
-        const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n1) - lo;
-        hash_children<false, true>(sA + 2 * lo, cnt, H, p.one);
-        digest_to_words(H, sB[2 * tid], sB[2 * tid + 1]);
-    }
-    __syncthreads();
-    if (n2 == 1) { if (tid < 2) root[tid] = sB[tid]; return; }
-    if (tid == 0) {
-        hash_children<false, true>(sB, n2, H, p.one);
-        digest_to_words(H, root[0], root[1]);
+    // One hash_children call site serves all (up to three) levels: the levels run one after the other on a nearly empty SM,
+    // so what counts is the length of the dependent chain and the amount of cold code, not throughput. Level sources and
+    // sinks are generic pointers (global input, then the two shared buffers).
+    const uint4 *src = reinterpret_cast<const uint4 *>(extra ? p.in2 : p.in + (size_t)t * p.in_tree_stride);
+    unsigned n = extra ? p.n_in2 : p.n_in;
+    uint4 *dst = sA;
+#pragma unroll 1
+    for (int level = 0; level < 3; ++level) {
+        const unsigned m = (n + FANOUT - 1) / FANOUT;
+        if (tid < m) {
+            const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n) - lo;
+            uint32_t H[8];
+            hash_children<false>(src + 2 * (size_t)lo, cnt, H, p.one);
+            uint4 a, b;
+            digest_to_words(H, a, b);
+            if (m == 1) { root[0] = a; root[1] = b; }
+            else { dst[2 * tid] = a; dst[2 * tid + 1] = b; }
+        }
+        if (m == 1) return;
+        __syncthreads();
+        src = dst; dst = (dst == sA) ? sB : sA; n = m;
     }
 }
 
@@ -130,8 +129,11 @@ struct StreamLeavesParams {
     uint32_t one;                  // = 1, opaque to the compiler (sha256_compress_rolled_fma)
 };
 
-__global__ void __launch_bounds__(HASH_THREADS) stream_leaves_kernel(const __grid_constant__ StreamLeavesParams p) {
-    const unsigned gid = blockIdx.x * HASH_THREADS + threadIdx.x;
+// 64-thread CTAs: a fragment of tens of MB has only tens of thousands of leaves (well under one full wave of the chip), so
+// small CTAs are what spreads them evenly over the SMs.
+constexpr int LEAF_THREADS = 64;
+__global__ void __launch_bounds__(LEAF_THREADS) stream_leaves_kernel(const __grid_constant__ StreamLeavesParams p) {
+    const unsigned gid = blockIdx.x * LEAF_THREADS + threadIdx.x;
     if (gid >= p.n_leaves[0] + p.n_leaves[1]) return;
     const int f = gid >= p.n_leaves[0] ? 1 : 0;
     const unsigned j = f ? gid - p.n_leaves[0] : gid;
