@@ -34,6 +34,8 @@ WORKLOADS = {
     "cfg2": ("dct", 1, 4096, 4096, 3, 5, 0, "BASELINE configs[1]: 4096x4096 RGB, k=5"),
     "cfg3": ("dct", 256, 1920, 1080, 3, 3, 16, "BASELINE configs[2]: batch of 256 RGB 1920x1080, k=3"),
     "cfg4": ("dwt", 1, 8192, 8192, 1, 3, 0, "BASELINE configs[3]: 8192x8192 gray, 3-level 5/3 DWT"),
+    # the sweep is not a bench line of its own: it prints one JSON line whose `sweep` array holds a point per (size, k | L)
+    "cfg5": ("sweep", 1, 0, 0, 3, 0, 0, "BASELINE configs[4]: square RGB 256^2..16384^2 x k in {0,2,5,9} (DCT) and L in {1,2,3,4} (DWT)"),
 }
 
 
@@ -137,6 +139,20 @@ def run_oracle_jobs(kind, jobs, kl, threads):
     return time.perf_counter() - t0, total
 
 
+def cpu_baseline_sample(kind, w, h, c, kl, target_s=12.0):
+    """The oracle as it stands on a bounded sample: one strip per host thread, passed over repeatedly until about
+    `target_s` seconds of wall time have gone by (first pass sizes the repeat count)."""
+    threads = min(os.cpu_count() or 1, 16)
+    rows = min(120 if kind == "dct" else 256, h)
+    jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
+    dt1, nbytes1 = run_oracle_jobs(kind, jobs, kl, threads)
+    passes = max(1, min(200, int(target_s / max(dt1, 1e-3))))
+    dt, nbytes = run_oracle_jobs(kind, jobs * passes, kl, threads)
+    return {"value": nbytes / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d passes over %d strips of %dx%dx%d (one strip per thread), fragment + verified defragment, %.1f s wall"
+                      % (passes, len(jobs), w, rows, c, dt)}
+
+
 def reference_arm(args, kind, n, w, h, c, kl, desc):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -164,6 +180,80 @@ def reference_arm(args, kind, n, w, h, c, kl, desc):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------------------------ cfg5 sweep
+def sweep_arm(args, desc):
+    """BASELINE configs[4]: fragment + verified defragment per point, device-resident, CUDA events; MB/s of image and the
+    algorithmic HBM GB/s (DCT: 5 B per pixel-channel and direction; DWT: 3 B) against the measured copy rate."""
+    import torch
+    import synth
+    from paper_1512_02951_b200 import binding as B
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    hbm_peak, _, peak_src = peaks()
+    key, nonce = synth.key_nonce(5)
+    points = []
+    sizes = [256, 512, 1024, 2048, 4096, 8192, 16384]
+    if args.images > 0:
+        sizes = [x for x in sizes if x <= args.images]   # --images N caps the edge length (quick runs)
+    for sz in sizes:
+        img = synth.image_batch_torch(1, sz, sz, 3, seed=5000 + sz, device=dev)
+        out = torch.empty_like(img)
+        nbytes = sz * sz * 3
+        reps = max(3, min(50, int(4e8 // nbytes)))
+        d_non = torch.from_numpy(__import__("numpy").frombuffer(nonce, dtype="uint8").copy()).to(dev).view(1, 16)
+        for k in [0, 2, 5, 9]:
+            batch = B.DctBatch(1, sz, sz, 3, k, device=dev)
+
+            def one():
+                batch.fragment(img, key, d_non)
+                batch.defragment(out, key, d_non, expected=batch.digests)
+            for _ in range(3):
+                one()
+            torch.cuda.synchronize()
+            assert torch.equal(out, img) and int(batch.flags_out.abs().sum().item()) == 0
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                one()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            points.append({"path": "dct", "size": sz, "k": k, "ms": ms, "MBps": nbytes / ms / 1e3, "hbm_GBps": nbytes * 10 / ms / 1e6,
+                           "hbm_frac": nbytes * 10 / ms / 1e6 / hbm_peak})
+            del batch
+        for L in [1, 2, 3, 4]:
+            ws = torch.empty(B.workspace_bytes(sz, sz, 3, L, True), dtype=torch.uint8, device=dev)
+            im = img[0]
+            st = {}
+
+            def one():
+                pv, pb, dg = B.fragment_dwt(im, L, key, nonce, workspace=ws)
+                st["rec"], st["fl"] = B.defragment_dwt(pv, pb, sz, sz, 3, L, key, nonce, expected=dg, workspace=ws)
+            for _ in range(3):
+                one()
+            torch.cuda.synchronize()
+            assert torch.equal(st["rec"], im) and int(st["fl"].item()) == 0
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                one()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            points.append({"path": "dwt", "size": sz, "levels": L, "ms": ms, "MBps": nbytes / ms / 1e3, "hbm_GBps": nbytes * 6 / ms / 1e6,
+                           "hbm_frac": nbytes * 6 / ms / 1e6 / hbm_peak})
+            del ws, st
+        del img, out
+        torch.cuda.empty_cache()
+    big = [p_ for p_ in points if p_["path"] == "dct" and p_["size"] == sizes[-1]]
+    line = {"metric": METRIC, "value": max(p_["MBps"] for p_ in big), "unit": UNIT, "n_gpus": 1, "steps": 0, "warmup": 3,
+            "ms_per_step": None, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32/int16", "data": "synthetic",
+            "config": {"workload": desc, "step": "fragment + verified defragment per point", "value_is": "best DCT point at the largest size",
+                       "l2": "points below 2048^2 fit the 126 MB L2: cached numbers", "hbm_peak_GBps": hbm_peak, "hbm_peak_source": peak_src},
+            "sweep": points}
+    print(json.dumps(line))
+
+
 # ------------------------------------------------------------------------------------------------------------ our arm
 def main():
     ap = argparse.ArgumentParser()
@@ -173,12 +263,21 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--images", type=int, default=0, help="override the number of images in the batch (DCT workloads)")
+    ap.add_argument("--k", type=int, default=-1, help="override k (DCT workloads) or the level count (DWT workload)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     kind, n, w, h, c, kl, rects, desc = WORKLOADS[args.workload]
     if args.images > 0 and kind == "dct":
         n = args.images
+    if args.k >= 0 and kind in ("dct", "dwt"):
+        kl = args.k
+        desc += " [k/levels overridden: %d]" % kl
+    if kind == "sweep":
+        if args.impl == "reference":
+            kind, n, w, h, c, kl, rects, desc = WORKLOADS["cfg2"]   # the oracle is timed on one mid-size point
+        else:
+            return sweep_arm(args, desc)
     if args.impl == "reference":
         return reference_arm(args, kind, n, w, h, c, kl, desc)
 
@@ -237,11 +336,21 @@ def main():
             nl_ = (nbytes + 2047) // 2048
             return tree_launch_count(nl_) - (1 if nl_ > 1 else 0)
         per_dig = 1 + wide(B.dwt_private_bytes(w, h, c, kl)) + wide(B.dwt_public_bytes(w, h, c, kl)) + 1
-        per_step_launches = (kl + 1 + per_dig) + (per_dig + 1 + 1 + kl)
+        per_step_launches = (kl + 1 + per_dig) + (per_dig + 1 + 1 + kl)   # levels + AES + digests | digests + compare + AES + levels
 
         def step(record=False):
+            if record:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                B.profile_events(e0, e1)
+                prof_frag.append((e0, e1))
             pv, pb, dg = B.fragment_dwt(d_img, kl, key, nonce, workspace=ws)
+            if record:
+                e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                B.profile_events(e2, e3)
+                prof_defrag.append((e2, e3))
             rec, fl = B.defragment_dwt(pv, pb, w, h, c, kl, key, nonce, expected=dg, workspace=ws)
+            if record:
+                B.profile_events(None, None)
             state["rec"], state["fl"] = rec, fl
             launches["n"] += per_step_launches
 
@@ -343,6 +452,63 @@ def main():
                               "fragment_hbm_GBps": core_bytes / (f_ms * 1e-3) / 1e9, "fragment_hbm_frac": core_bytes / (f_ms * 1e-3) / 1e9 / hbm_peak,
                               "defragment_hbm_GBps": core_bytes / (d_ms * 1e-3) / 1e9, "defragment_hbm_frac": core_bytes / (d_ms * 1e-3) / 1e9 / hbm_peak}
 
+    if kind == "dwt":
+        # dominant kernel: stream_leaves_kernel (SHA-256 of every 2048-byte leaf of both fragments), ALU-bound like the DCT path
+        pvb, pbb = B.dwt_private_bytes(w, h, c, kl), B.dwt_public_bytes(w, h, c, kl)
+
+        def comps(nbytes):   # compressions: full leaves take 33, the last leaf ceil((len + 9) / 64)
+            full, tail = divmod(nbytes, 2048)
+            return full * 33 + ((tail + 9 + 63) // 64 if tail else 0)
+        leaf_ms = statistics.mean(a.elapsed_time(b_) for a, b_ in prof_frag + prof_defrag)
+        alu_ops = (comps(pvb) + comps(pbb)) * 1040.0
+        alu_peak = 148 * 64 * sm_max_mhz * 1e6 / 1e12
+        achieved = alu_ops / (leaf_ms * 1e-3) / 1e12
+        nleaves = (pvb + 2047) // 2048 + (pbb + 2047) // 2048
+        alg_bytes = pvb + pbb + 32 * nleaves
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+        if os.path.exists(tpath):
+            traffic = json.load(open(tpath)).get("stream_leaves_kernel@%s/%d" % (args.workload, n))
+        roofline = {"kernel": "stream_leaves_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                    "unit": "Tlane-op/s (32-bit ops only the ALU pipe executes: SHF/LOP3/PRMT)", "frac": achieved / alu_peak,
+                    "peak_source": "derived: 148 SM x 64 ALU-pipe lanes/clk x %.0f MHz (DESIGN.md section 7)" % sm_max_mhz,
+                    "algorithmic_ops_per_launch": alu_ops, "traffic": traffic, "ms_per_launch": leaf_ms,
+                    "hbm_view": {"achieved": alg_bytes / (leaf_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                 "frac": alg_bytes / (leaf_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src,
+                                 "algorithmic_bytes_per_launch": alg_bytes}}
+        stages["leaf_hash_kernel_GBps_hashed"] = (pvb + pbb) / (leaf_ms * 1e-3) / 1e9
+
+    # the two cryptographic steps alone on a long stream (north_star: "AES reported separately as GB/s against its integer-ALU
+    # bound"); the AES call on the image bytes is also the report's full-image AES baseline
+    if rank == 0:
+        src = d_imgs.view(-1) if kind == "dct" else d_img.view(-1)
+        dst = torch.empty_like(src)
+        mws = torch.empty(max(16, B.lib.feds_sha256_merkle_workspace_bytes(src.numel())), dtype=torch.uint8, device=dev)
+        for _ in range(2):
+            B.aes128_ctr(src, key, nonce, out=dst)
+            B.sha256_merkle(src, workspace=mws)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        reps = 5
+        ev[0].record()
+        for _ in range(reps):
+            B.aes128_ctr(src, key, nonce, out=dst)
+        ev[1].record()
+        for _ in range(reps):
+            B.sha256_merkle(src, workspace=mws)
+        ev[2].record()
+        torch.cuda.synchronize()
+        a_ms, s_ms = ev[0].elapsed_time(ev[1]) / reps, ev[1].elapsed_time(ev[2]) / reps
+        alu_peak = 148 * 64 * sm_max_mhz * 1e6   # lane-ops/s
+        aes_bound = alu_peak / (250.0 / 16.0) / 1e9     # 250 ALU-pipe ops per 16-byte block
+        sha_bound = alu_peak / (1040.0 * 33 / 2048.0) / 1e9   # 33 compressions of 1040 ALU-pipe ops per 2048-byte leaf
+        stages["aes128_ctr_stream"] = {"bytes": src.numel(), "GBps": src.numel() / (a_ms * 1e-3) / 1e9, "alu_bound_GBps": aes_bound,
+                                       "frac_of_alu_bound": src.numel() / (a_ms * 1e-3) / 1e9 / aes_bound,
+                                       "note": "out-of-place over the whole input: the report's full-image AES baseline"}
+        stages["sha256_merkle_stream"] = {"bytes": src.numel(), "GBps": src.numel() / (s_ms * 1e-3) / 1e9, "alu_bound_GBps": sha_bound,
+                                          "frac_of_alu_bound": src.numel() / (s_ms * 1e-3) / 1e9 / sha_bound}
+        del dst, mws
+
     # ---------------------------------------------------------------- end to end through the host-buffer C ABI
     e2e = None
     if kind == "dct" and not args.no_e2e:
@@ -422,12 +588,7 @@ def main():
     # ---------------------------------------------------------------- CPU oracle baseline (rank 0, N = 1 only)
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        threads = min(os.cpu_count() or 1, 16)
-        rows = min(120 if kind == "dct" else 256, h)
-        jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
-        dt, nbytes = run_oracle_jobs(kind, jobs, kl, threads)
-        cpu_baseline = {"value": nbytes / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
-                        "sample": "%d strips of %dx%dx%d (one per thread), fragment + verified defragment, %.1f s wall" % (len(jobs), w, rows, c, dt)}
+        cpu_baseline = cpu_baseline_sample(kind, w, h, c, kl)
 
     if rank == 0:
         line = {

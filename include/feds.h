@@ -173,8 +173,9 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
                                size_t workspace_bytes, feds_stream_t stream);
 
 /*
- * Profiling hook (not part of the data path; thread-local): while set, every DCT fragment/defragment call made on this
- * thread records ev_start immediately before and ev_stop immediately after its fused tile kernel, on the call's stream.
+ * Profiling hook (not part of the data path; thread-local): while set, every fragment/defragment call made on this
+ * thread records ev_start immediately before and ev_stop immediately after its dominant kernel, on the call's stream:
+ * the fused tile kernel of the DCT path, the leaf-hashing kernel of the DWT path.
  * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.
  */
 void feds_profile_events(void *ev_start, void *ev_stop);

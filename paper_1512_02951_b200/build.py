@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.environ.get("FEDS_LIB_PATH") or os.path.join(HERE, "libfeds.so")
 SOURCES = ["feds_api.cu"]
-HEADERS = ["feds_device.cuh", "feds_dct.cuh", "feds_hash.cuh", "feds_dwt.cuh", "feds_dwt_fast.cuh", "feds_peaks.cu", os.path.join("..", "..", "include", "feds.h")]
+HEADERS = ["feds_device.cuh", "feds_dct.cuh", "feds_dct_tile.cuh", "feds_hash.cuh", "feds_dwt.cuh", "feds_dwt_fast.cuh", "feds_peaks.cu", os.path.join("..", "..", "include", "feds.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

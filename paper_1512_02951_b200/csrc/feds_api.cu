@@ -9,6 +9,7 @@
 
 #include "../../include/feds.h"
 #include "feds_dct.cuh"
+#include "feds_dct_tile.cuh"
 #include "feds_device.cuh"
 #include "feds_dwt.cuh"
 #include "feds_dwt_fast.cuh"
@@ -202,10 +203,29 @@ feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream, i
     return FEDS_OK;
 }
 
+// digest-free path: persistent tile kernels, as many CTAs per SM as fit (feds_dct_tile.cuh)
+template <int C, typename Kernel>
+feds_status launch_dct_tile(Kernel kernel, const DctParams &p, cudaStream_t stream) {
+    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB;
+    const size_t smem = tile_smem_bytes<C>(p.k);
+    feds_status s = set_smem(kernel, smem);
+    if (s != FEDS_OK) return s;
+    int per_sm = 0;
+    FEDS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, THREADS, smem));
+    if (per_sm < 1) per_sm = 1;
+    const unsigned long long tiles = (unsigned long long)p.n_images * p.nbr * ((p.nbc + TB - 1) / TB);
+    const unsigned grid = (unsigned)std::min<unsigned long long>(tiles, (unsigned long long)per_sm * sm_count());
+    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
+    kernel<<<grid, THREADS, smem, stream>>>(p);
+    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
 template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, true>, p, s); } };
-template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, false>, p, s); } };
+template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(fragment_dct_tile_kernel<C, V>, p, s); } };
 template <int C, int V> struct DefragVerify { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, true>, p, s, DEFRAG_THREADS); } };
-template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(defragment_dct_kernel<C, V, false>, p, s, DEFRAG_THREADS); } };
+template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(defragment_dct_tile_kernel<C, V>, p, s); } };
 
 template <bool DIGEST>
 feds_status launch_fragment(const DctParams &p, int c, cudaStream_t stream) {
@@ -391,7 +411,9 @@ feds_status dwt_digests(const uint8_t *d_private, const uint8_t *d_public, const
         sp.out[f] = nls[f] > 1 ? ws[f] : roots + 32 * f;  // a one-leaf fragment's root is its leaf digest
     }
     const unsigned total = nls[0] + nls[1];
+    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
     stream_leaves_kernel<<<(total + LEAF_THREADS - 1) / LEAF_THREADS, LEAF_THREADS, 0, stream>>>(sp);
+    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
     FEDS_LAUNCH_CHECK();
     return run_two_trees(ws[0], nls[0], ws[0] + (size_t)nls[0] * 32, roots, ws[1], nls[1], ws[1] + (size_t)nls[1] * 32, roots + 32, stream);
 }

@@ -246,3 +246,37 @@ def test_config3_batch_full_size(orc, b):
     # every image's digests are distinct (independent CTR messages, A20)
     dgs = batch.digests.cpu().numpy().reshape(n, 64)
     assert len({bytes(r[:32]) for r in dgs}) == n
+
+
+# the digest-free path runs different kernels (persistent tile kernels, feds_dct_tile.cuh): same arithmetic, other data movement
+@pytest.mark.parametrize("n,w,h,c,k", [(1, 8, 8, 1, 0), (1, 8, 8, 1, 63), (2, 264, 16, 3, 3), (1, 1032, 24, 1, 5), (3, 1920, 16, 3, 3),
+                                       (1, 4104, 8, 1, 2), (2, 520, 40, 4, 7), (1, 776, 8, 3, 0), (1, 256, 64, 3, 9), (1, 512, 8, 4, 62),
+                                       (1, 2048, 8, 3, 31), (1, 2048, 8, 3, 32)])
+def test_digest_free_tile_kernels(orc, b, n, w, h, c, k):
+    key, nonce = synth.key_nonce(w + k)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=7 * w + i + k, rectangles=1 if w >= 64 and h >= 16 else 0) for i in range(n)])
+    d_imgs = torch.from_numpy(imgs).cuda()
+    d_nonces = torch.from_numpy(nonces).cuda()
+    full, plain = b.DctBatch(n, w, h, c, k), b.DctBatch(n, w, h, c, k)
+    for t in (full.priv, full.pub, plain.priv, plain.pub):
+        t.fill_(0xA5)   # torch.empty may hand back a buffer that already holds the right bytes
+    full.fragment(d_imgs, key, d_nonces)
+    plain.fragment(d_imgs, key, d_nonces, flags=b.FLAG_NO_DIGEST)
+    torch.cuda.synchronize()
+    assert torch.equal(plain.priv, full.priv), "private fragments differ"
+    assert torch.equal(plain.pub, full.pub), "public fragments differ"
+    # stage (i)/(ii) against the oracle on the tile kernels' own output, image 0
+    pv = plain.priv[:plain.priv_bytes].cpu().numpy()
+    pb = plain.pub[:plain.pub_bytes].cpu().numpy()
+    coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[0].tobytes())
+    assert np.abs(coef - orc.dct_coefficients(imgs[0])).max() <= TOL
+    p2, q2, _ = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[0].tobytes())
+    assert (p2 == pv).all() and (q2 == pb).all()
+    # inverse without verification: tile kernel; with verification: fused kernel; both exact
+    out = torch.zeros_like(d_imgs)
+    plain.defragment(out, key, d_nonces)
+    assert torch.equal(out, d_imgs)
+    out.zero_()
+    full.defragment(out, key, d_nonces, expected=full.digests)
+    assert torch.equal(out, d_imgs) and int(full.flags_out.abs().sum().item()) == 0
