@@ -203,20 +203,17 @@ feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream, i
     return FEDS_OK;
 }
 
-// digest-free path: persistent tile kernels, as many CTAs per SM as fit (feds_dct_tile.cuh)
+// digest-free path: one persistent CTA per SM, GROUPS tile groups inside it (feds_dct_tile.cuh)
 template <int C, typename Kernel>
 feds_status launch_dct_tile(Kernel kernel, const DctParams &p, cudaStream_t stream) {
-    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB;
+    constexpr int TB = TileShape<C>::TB, GROUPS = TileShape<C>::GROUPS;
     const size_t smem = tile_smem_bytes<C>(p.k);
     feds_status s = set_smem(kernel, smem);
     if (s != FEDS_OK) return s;
-    int per_sm = 0;
-    FEDS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, THREADS, smem));
-    if (per_sm < 1) per_sm = 1;
     const unsigned long long tiles = (unsigned long long)p.n_images * p.nbr * ((p.nbc + TB - 1) / TB);
-    const unsigned grid = (unsigned)std::min<unsigned long long>(tiles, (unsigned long long)per_sm * sm_count());
+    const unsigned grid = (unsigned)std::min<unsigned long long>((tiles + GROUPS - 1) / GROUPS, (unsigned long long)sm_count());
     if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    kernel<<<grid, THREADS, smem, stream>>>(p);
+    kernel<<<grid, TileShape<C>::CTA, smem, stream>>>(p);
     if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;

@@ -94,22 +94,25 @@ __device__ __forceinline__ void vec_load_global(const uint32_t *src, uint32_t (&
     else { const uint4 t = __ldg(reinterpret_cast<const uint4 *>(src)); x[0] = t.x; x[1 % V] = t.y; x[2 % V] = t.z; x[3 % V] = t.w; }
 }
 
-template <int C>
+template <typename T, bool GLOBAL>
+__device__ __forceinline__ T ld_ro(const T *q) { return GLOBAL ? __ldg(q) : *q; }
+// GLOBAL = false: `img` is a tile of pixel rows staged in shared memory (same interleaved layout, pitch w pixels)
+template <int C, bool GLOBAL = true>
 __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int w, int y0, int x0, int c, float (&v)[64]) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const uint8_t *row = img + ((size_t)(y0 + r) * w + x0) * C;
         if (C == 1) {
-            const uint2 q = __ldg(reinterpret_cast<const uint2 *>(row));
+            const uint2 q = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row));
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 v[8 * r + i] = (float)((q.x >> (8 * i)) & 0xffu);
                 v[8 * r + 4 + i] = (float)((q.y >> (8 * i)) & 0xffu);
             }
         } else if (C == 3) {
-            const uint2 q0 = __ldg(reinterpret_cast<const uint2 *>(row));
-            const uint2 q1 = __ldg(reinterpret_cast<const uint2 *>(row) + 1);
-            const uint2 q2 = __ldg(reinterpret_cast<const uint2 *>(row) + 2);
+            const uint2 q0 = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row));
+            const uint2 q1 = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row) + 1);
+            const uint2 q2 = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row) + 2);
             // shift the 24-byte row right by c bytes (c is fixed per thread), then the wanted bytes sit at 3*i
             const uint32_t wd[7] = {q0.x, q0.y, q1.x, q1.y, q2.x, q2.y, 0u};
             uint32_t ws[6];
@@ -118,8 +121,8 @@ __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int 
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[8 * r + i] = (float)((ws[(3 * i) >> 2] >> (8 * ((3 * i) & 3))) & 0xffu);
         } else {
-            const uint4 a = __ldg(reinterpret_cast<const uint4 *>(row));
-            const uint4 b = __ldg(reinterpret_cast<const uint4 *>(row) + 1);
+            const uint4 a = ld_ro<uint4, GLOBAL>(reinterpret_cast<const uint4 *>(row));
+            const uint4 b = ld_ro<uint4, GLOBAL>(reinterpret_cast<const uint4 *>(row) + 1);
             const uint32_t wd[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
             const int sh = 8 * c;
 #pragma unroll
@@ -367,8 +370,8 @@ struct Keystream {
     uint32_t ks[4];
     unsigned long long blk;
 };
-template <int V>
-__device__ __forceinline__ void keystream_words(Keystream &K, const uint32_t *sT, const uint32_t *rk, const uint32_t (&nonce)[4],
+template <int V, typename Tab>
+__device__ __forceinline__ void keystream_words(Keystream &K, const Tab sT, const uint32_t *rk, const uint32_t (&nonce)[4],
                                                 unsigned long long wi, uint32_t (&out)[V]) {
     const unsigned long long blk = wi >> 2;
     if (V == 4 || blk != K.blk) {

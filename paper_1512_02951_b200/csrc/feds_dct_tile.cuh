@@ -6,20 +6,49 @@
 //   in 64 registers. The fragments of the tile are staged in shared memory in exactly their global byte order (the public
 //   runs of consecutive blocks of one channel are contiguous), so the traffic with HBM is a flat,
 //   fully coalesced 128-bit copy in both directions; AES-128-CTR is applied to the private words on their way through.
-//   CTAs are persistent (the AES tables are filled once) and several share an SM, which overlaps one tile's loads with
-//   another's arithmetic and stores.
+//   One persistent CTA per SM holds GROUPS independent thread groups (3-4 warps each, synchronised with their own named
+//   barrier), each working on its own tile with its own stage, so one tile's loads overlap another's arithmetic and
+//   stores. The groups share one AES table: T0 only, each entry replicated 32 times so that lane l reads copy l, which
+//   lies in bank l -- every lookup is conflict-free (random lookups in a plain 4 KB table set collide ~3.4-fold and
+//   were measured to cost a third of the kernel's time); T1..T3 are byte rotations of T0.
 #pragma once
 #include "feds_dct.cuh"
 
 namespace feds {
 
-template <int C> struct TileShape { static constexpr int THREADS = (C == 3) ? 96 : 128, TB = THREADS / C; };
+template <int C> struct TileShape {
+    static constexpr int THREADS = (C == 3) ? 96 : 128;   // per group
+    static constexpr int TB = THREADS / C;                // blocks per tile and channel
+    static constexpr int GROUPS = (C == 3) ? 6 : 4;
+    static constexpr int CTA = THREADS * GROUPS;
+};
+constexpr int T0_REPL = 32, T0_WORDS = 256 * T0_REPL;
 // Words between the staged runs of two channels: the smallest count >= words that is 20 mod 32, so that the C lanes of one
 // block column (adjacent lanes) and their neighbours land in different banks when they write their runs with 128-bit stores.
 __host__ __device__ inline int tile_run_stride(int words) { return ((words + 11) / 32) * 32 + 20; }
-template <int C> __host__ __device__ inline size_t tile_smem_bytes(int k) {
-    return (size_t)(AES_TABLE_WORDS + C * (tile_run_stride(TileShape<C>::TB * (63 - k)) + tile_run_stride(TileShape<C>::TB * (k + 1)))) * 4;
+// words of one group's shared memory: the two staged fragments
+template <int C> __host__ __device__ inline int tile_group_words(int k) {
+    return C * (tile_run_stride(TileShape<C>::TB * (63 - k)) + tile_run_stride(TileShape<C>::TB * (k + 1)));
 }
+template <int C> __host__ __device__ inline size_t tile_smem_bytes(int k) {
+    return (size_t)(T0_WORDS + TileShape<C>::GROUPS * tile_group_words<C>(k)) * 4;
+}
+
+// Entry t*256 + x of the four FIPS-197 round tables, served from the lane's own copies of T0 (b = table + lane).
+struct T0Lane {
+    const uint32_t *b;
+    __device__ __forceinline__ uint32_t operator[](unsigned i) const {
+        const uint32_t v = b[(i & 255u) * T0_REPL];
+        const unsigned t = i >> 8;   // a compile-time constant at every call site of aes128_encrypt
+        return t == 0 ? v : t == 1 ? __funnelshift_l(v, v, 8) : t == 2 ? __funnelshift_l(v, v, 16) : __funnelshift_l(v, v, 24);
+    }
+};
+__device__ __forceinline__ void load_t0_replicated(uint32_t *sTab) {
+    const uint32_t *src = &g_aes.T[0][0];
+    for (int i = threadIdx.x; i < T0_WORDS; i += blockDim.x) sTab[i] = src[i / T0_REPL];
+    __syncthreads();
+}
+__device__ __forceinline__ void group_sync(int gid, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(gid + 1), "r"(nthreads) : "memory"); }
 
 struct TileCoord {
     int n, br, bc0, nb;  // image, block row, first block column, blocks in the tile
@@ -40,42 +69,80 @@ __device__ __forceinline__ TileCoord decode_tile(const DctParams &p, unsigned t,
 // Global -> shared goes through cp.async (LDGSTS): no register staging, every thread keeps all of its 16-byte pieces in
 // flight at once; the caller waits with tile_copy_wait() before the barrier.
 template <bool TO_GLOBAL, int THREADS>
-__device__ __forceinline__ void tile_copy(uint32_t *g, uint32_t *s, int words) {
+__device__ __forceinline__ void tile_copy(uint32_t *g, uint32_t *s, int words, int tid) {
     if (((reinterpret_cast<uintptr_t>(g) & 15u) == 0) && ((words & 3) == 0)) {
         uint4 *g4 = reinterpret_cast<uint4 *>(g);
         uint4 *s4 = reinterpret_cast<uint4 *>(s);
         if (TO_GLOBAL) {
-            for (int i = threadIdx.x; i < (words >> 2); i += THREADS) g4[i] = s4[i];
+            for (int i = tid; i < (words >> 2); i += THREADS) g4[i] = s4[i];
         } else {
             const uint32_t sa = (uint32_t)__cvta_generic_to_shared(s4);
-            for (int i = threadIdx.x; i < (words >> 2); i += THREADS)
+            for (int i = tid; i < (words >> 2); i += THREADS)
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa + 16u * i), "l"(g4 + i) : "memory");
         }
     } else {
-        for (int i = threadIdx.x; i < words; i += THREADS) {
+        for (int i = tid; i < words; i += THREADS) {
             if (TO_GLOBAL) g[i] = s[i]; else s[i] = __ldg(g + i);
         }
     }
 }
 __device__ __forceinline__ void tile_copy_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
+// AES-128-CTR over the staged private runs of a tile, by the whole group: every 16-byte counter block that overlaps a run
+// is computed once, by one thread, whatever k is (a thread that followed its own block's words would compute 2-3 AES
+// blocks per 8x8 block whenever 4 does not divide k + 1). Run c holds words [W0_c, W0_c + nw) of the image's private stream.
+template <int C, int THREADS>
+__device__ __forceinline__ void tile_aes_ctr(const DctParams &p, const T0Lane &sT, const TileCoord &T, uint32_t *s_priv, int RSP, int P, int tid) {
+    uint32_t nonce[4];
+    load_nonce(p, T.n, nonce);
+    const int nw = T.nb * P;
+    const int per = (TileShape<C>::TB * P + 3) / 4 + 1;   // >= counter blocks overlapping one run
+    for (int idx = tid; idx < C * per; idx += THREADS) {
+        const int c = idx / per, i = idx % per;
+        const unsigned long long W0 = ((unsigned long long)(c * p.nbr + T.br) * p.nbc + T.bc0) * P;
+        const unsigned long long blk = (W0 >> 2) + i;
+        const long long first = (long long)(blk << 2) - (long long)W0;   // run-relative index of the block's first word
+        if (first >= nw) continue;
+        uint32_t ks[4];
+        ctr_block(nonce, blk, ks);
+        aes128_encrypt(sT, p.rk, ks);
+        uint32_t *run = s_priv + c * RSP;
+        if (first >= 0 && first + 4 <= nw) {
+            uint4 *q = reinterpret_cast<uint4 *>(run + first);   // first is a multiple of 4 here iff W0 is: else fall through
+            if ((first & 3) == 0) {
+                uint4 x = *q;
+                x.x ^= ks[0]; x.y ^= ks[1]; x.z ^= ks[2]; x.w ^= ks[3];
+                *q = x;
+                continue;
+            }
+        }
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const long long r = first + w;
+            if (r >= 0 && r < nw) run[r] ^= ks[w];
+        }
+    }
+}
+
 // Stage layout (words): [AES tables 1024][public: C runs of TB*Q, tile_run_stride apart][private: C runs of TB*P likewise];
 // every run starts 16-byte aligned.
 template <int C, int V>
-__global__ void __launch_bounds__(TileShape<C>::THREADS) fragment_dct_tile_kernel(const __grid_constant__ DctParams p) {
-    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB;
+__global__ void __launch_bounds__(TileShape<C>::CTA, 1) fragment_dct_tile_kernel(const __grid_constant__ DctParams p) {
+    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB, GROUPS = TileShape<C>::GROUPS;
     extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *sT = smem;
-    load_aes_tables(sT);
+    load_t0_replicated(smem);
+    T0Lane sT;
+    sT.b = smem + (threadIdx.x & 31);
     constexpr ZigzagTable ZZ = make_zigzag();
     const int k = p.k, P = k + 1, Q = 63 - k;
     const int RSQ = tile_run_stride(TB * Q), RSP = tile_run_stride(TB * P);
-    uint32_t *s_pub = smem + AES_TABLE_WORDS, *s_priv = s_pub + C * RSQ;
-    const int j = threadIdx.x / C, ch = threadIdx.x % C;
+    const int gid = threadIdx.x / THREADS, tid = threadIdx.x % THREADS;
+    uint32_t *s_pub = smem + T0_WORDS + gid * tile_group_words<C>(k), *s_priv = s_pub + C * RSQ;
+    const int j = tid / C, ch = tid % C;
     const int tiles_per_row = (p.nbc + TB - 1) / TB;
     const unsigned total = (unsigned)p.n_images * p.nbr * tiles_per_row;
 #pragma unroll 1
-    for (unsigned t = blockIdx.x; t < total; t += gridDim.x) {
+    for (unsigned t = blockIdx.x * GROUPS + gid; t < total; t += gridDim.x * GROUPS) {
         const TileCoord T = decode_tile<C>(p, t, tiles_per_row);
         const bool act = j < T.nb;
         uint32_t *my_pub = s_pub + ch * RSQ + j * Q - P;  // indexed by z
@@ -84,11 +151,6 @@ __global__ void __launch_bounds__(TileShape<C>::THREADS) fragment_dct_tile_kerne
             float v[64];
             load_block<C>(p.images + (size_t)T.n * p.image_stride, p.w, 8 * T.br, 8 * (T.bc0 + j), ch, v);
             dct8x8(v);
-            uint32_t nonce[4];
-            load_nonce(p, T.n, nonce);
-            Keystream K;
-            K.blk = ~0ull;
-            const unsigned long long w0 = ((unsigned long long)(ch * p.nbr + T.br) * p.nbc + T.bc0 + j) * P;
 #pragma unroll
             for (int g = 0; g < 64; g += V) {
                 uint32_t x[V];
@@ -96,69 +158,88 @@ __global__ void __launch_bounds__(TileShape<C>::THREADS) fragment_dct_tile_kerne
                 for (int q = 0; q < V; ++q) x[q] = __float_as_uint(v[ZZ.pos[g + q]]);
                 vec_store<V>(g < P ? my_priv + g : my_pub + g, x);
             }
+            if (V == 4) {   // 4 | k + 1: the block's private words are whole counter blocks of their own -- encrypt them here
+                uint32_t nonce[4];
+                load_nonce(p, T.n, nonce);
+                const unsigned long long w0 = ((unsigned long long)(ch * p.nbr + T.br) * p.nbc + T.bc0 + j) * P;
 #pragma unroll 1
-            for (int g = 0; g < P; g += V) {   // AES-128-CTR on the private words, in place in the stage
-                uint32_t ks[V], x[V];
-                keystream_words<V>(K, sT, p.rk, nonce, w0 + g, ks);
-                vec_load<V>(my_priv + g, x);
-#pragma unroll
-                for (int q = 0; q < V; ++q) x[q] ^= ks[q];
-                vec_store<V>(my_priv + g, x);
+                for (int g = 0; g < P; g += 4) {
+                    uint32_t ks[4];
+                    ctr_block(nonce, (w0 + g) >> 2, ks);
+                    aes128_encrypt(sT, p.rk, ks);
+                    uint4 x = *reinterpret_cast<uint4 *>(my_priv + g);
+                    x.x ^= ks[0]; x.y ^= ks[1]; x.z ^= ks[2]; x.w ^= ks[3];
+                    *reinterpret_cast<uint4 *>(my_priv + g) = x;
+                }
             }
         }
-        __syncthreads();
+        group_sync(gid, THREADS);
+#pragma unroll
+        for (int c = 0; c < C; ++c) {   // the public runs leave first; their stores drain while the private runs are encrypted
+            const size_t b0 = (size_t)(c * p.nbr + T.br) * p.nbc + T.bc0;
+            tile_copy<true, THREADS>(reinterpret_cast<uint32_t *>(p.pub + (size_t)T.n * p.pub_stride) + b0 * Q, s_pub + c * RSQ, T.nb * Q, tid);
+        }
+        if (V != 4) {
+            tile_aes_ctr<C, THREADS>(p, sT, T, s_priv, RSP, P, tid);
+            group_sync(gid, THREADS);
+        }
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             const size_t b0 = (size_t)(c * p.nbr + T.br) * p.nbc + T.bc0;
-            tile_copy<true, THREADS>(reinterpret_cast<uint32_t *>(p.pub + (size_t)T.n * p.pub_stride) + b0 * Q, s_pub + c * RSQ, T.nb * Q);
-            tile_copy<true, THREADS>(reinterpret_cast<uint32_t *>(p.priv + (size_t)T.n * p.priv_stride) + b0 * P, s_priv + c * RSP, T.nb * P);
+            tile_copy<true, THREADS>(reinterpret_cast<uint32_t *>(p.priv + (size_t)T.n * p.priv_stride) + b0 * P, s_priv + c * RSP, T.nb * P, tid);
         }
-        __syncthreads();
+        group_sync(gid, THREADS);
     }
 }
 
 template <int C, int V>
-__global__ void __launch_bounds__(TileShape<C>::THREADS) defragment_dct_tile_kernel(const __grid_constant__ DctParams p) {
-    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB;
+__global__ void __launch_bounds__(TileShape<C>::CTA, 1) defragment_dct_tile_kernel(const __grid_constant__ DctParams p) {
+    constexpr int THREADS = TileShape<C>::THREADS, TB = TileShape<C>::TB, GROUPS = TileShape<C>::GROUPS;
     extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *sT = smem;
-    load_aes_tables(sT);
+    load_t0_replicated(smem);
+    T0Lane sT;
+    sT.b = smem + (threadIdx.x & 31);
     constexpr ZigzagTable ZZ = make_zigzag();
     const int k = p.k, P = k + 1, Q = 63 - k;
     const int RSQ = tile_run_stride(TB * Q), RSP = tile_run_stride(TB * P);
-    uint32_t *s_pub = smem + AES_TABLE_WORDS, *s_priv = s_pub + C * RSQ;
-    const int j = threadIdx.x / C, ch = threadIdx.x % C;
+    const int gid = threadIdx.x / THREADS, tid = threadIdx.x % THREADS;
+    uint32_t *s_pub = smem + T0_WORDS + gid * tile_group_words<C>(k), *s_priv = s_pub + C * RSQ;
+    const int j = tid / C, ch = tid % C;
     const int tiles_per_row = (p.nbc + TB - 1) / TB;
     const unsigned total = (unsigned)p.n_images * p.nbr * tiles_per_row;
 #pragma unroll 1
-    for (unsigned t = blockIdx.x; t < total; t += gridDim.x) {
+    for (unsigned t = blockIdx.x * GROUPS + gid; t < total; t += gridDim.x * GROUPS) {
         const TileCoord T = decode_tile<C>(p, t, tiles_per_row);
         const bool act = j < T.nb;
 #pragma unroll
         for (int c = 0; c < C; ++c) {
             const size_t b0 = (size_t)(c * p.nbr + T.br) * p.nbc + T.bc0;
-            tile_copy<false, THREADS>(reinterpret_cast<uint32_t *>(p.pub + (size_t)T.n * p.pub_stride) + b0 * Q, s_pub + c * RSQ, T.nb * Q);
-            tile_copy<false, THREADS>(reinterpret_cast<uint32_t *>(p.priv + (size_t)T.n * p.priv_stride) + b0 * P, s_priv + c * RSP, T.nb * P);
+            tile_copy<false, THREADS>(reinterpret_cast<uint32_t *>(p.pub + (size_t)T.n * p.pub_stride) + b0 * Q, s_pub + c * RSQ, T.nb * Q, tid);
+            tile_copy<false, THREADS>(reinterpret_cast<uint32_t *>(p.priv + (size_t)T.n * p.priv_stride) + b0 * P, s_priv + c * RSP, T.nb * P, tid);
         }
         tile_copy_wait();
-        __syncthreads();
+        group_sync(gid, THREADS);
+        if (V != 4) {
+            tile_aes_ctr<C, THREADS>(p, sT, T, s_priv, RSP, P, tid);
+            group_sync(gid, THREADS);
+        }
         float v[64];
         if (act) {
             uint32_t *my_pub = s_pub + ch * RSQ + j * Q - P;  // indexed by z
             uint32_t *my_priv = s_priv + ch * RSP + j * P;
-            uint32_t nonce[4];
-            load_nonce(p, T.n, nonce);
-            Keystream K;
-            K.blk = ~0ull;
-            const unsigned long long w0 = ((unsigned long long)(ch * p.nbr + T.br) * p.nbc + T.bc0 + j) * P;
+            if (V == 4) {   // decrypt this block's own counter blocks in place
+                uint32_t nonce[4];
+                load_nonce(p, T.n, nonce);
+                const unsigned long long w0 = ((unsigned long long)(ch * p.nbr + T.br) * p.nbc + T.bc0 + j) * P;
 #pragma unroll 1
-            for (int g = 0; g < P; g += V) {   // decrypt in place in the stage
-                uint32_t ks[V], x[V];
-                keystream_words<V>(K, sT, p.rk, nonce, w0 + g, ks);
-                vec_load<V>(my_priv + g, x);
-#pragma unroll
-                for (int q = 0; q < V; ++q) x[q] ^= ks[q];
-                vec_store<V>(my_priv + g, x);
+                for (int g = 0; g < P; g += 4) {
+                    uint32_t ks[4];
+                    ctr_block(nonce, (w0 + g) >> 2, ks);
+                    aes128_encrypt(sT, p.rk, ks);
+                    uint4 x = *reinterpret_cast<uint4 *>(my_priv + g);
+                    x.x ^= ks[0]; x.y ^= ks[1]; x.z ^= ks[2]; x.w ^= ks[3];
+                    *reinterpret_cast<uint4 *>(my_priv + g) = x;
+                }
             }
 #pragma unroll
             for (int g = 0; g < 64; g += V) {
@@ -170,7 +251,7 @@ __global__ void __launch_bounds__(TileShape<C>::THREADS) defragment_dct_tile_ker
             idct8x8(v);
         }
         store_block<C>(p.images_out + (size_t)T.n * p.image_stride, p.w, 8 * T.br, 8 * (T.bc0 + j), ch, act, v);
-        __syncthreads();
+        group_sync(gid, THREADS);
     }
 }
 
