@@ -34,15 +34,40 @@ template <int C> __host__ __device__ inline size_t tile_smem_bytes(int k) {
     return (size_t)(T0_WORDS + TileShape<C>::GROUPS * tile_group_words<C>(k)) * 4;
 }
 
-// Entry t*256 + x of the four FIPS-197 round tables, served from the lane's own copies of T0 (b = table + lane).
+// AES-128 rounds on the lane's own copies of T0 (copy l of entry x at byte x * 128 + l * 4; lane4 = 4 * lane): every lookup
+// is shift, mask-and-or-in-the-lane, LDS, and for T1..T3 one byte rotation of the T0 word. Same arithmetic as aes128_encrypt.
 struct T0Lane {
-    const uint32_t *b;
-    __device__ __forceinline__ uint32_t operator[](unsigned i) const {
-        const uint32_t v = b[(i & 255u) * T0_REPL];
-        const unsigned t = i >> 8;   // a compile-time constant at every call site of aes128_encrypt
-        return t == 0 ? v : t == 1 ? __funnelshift_l(v, v, 8) : t == 2 ? __funnelshift_l(v, v, 16) : __funnelshift_l(v, v, 24);
-    }
+    const char *tab;
+    uint32_t lane4;
 };
+template <int BYTE, int TABLE>
+__device__ __forceinline__ uint32_t t0_lookup(const T0Lane &T, uint32_t word) {
+    uint32_t o;
+    if (BYTE == 0) o = ((word << 7) & 0x7f80u) | T.lane4;
+    else if (BYTE == 1) o = ((word >> 1) & 0x7f80u) | T.lane4;
+    else if (BYTE == 2) o = ((word >> 9) & 0x7f80u) | T.lane4;
+    else o = ((word >> 17) & 0x7f80u) | T.lane4;
+    const uint32_t v = *reinterpret_cast<const uint32_t *>(T.tab + o);
+    return TABLE == 0 ? v : __funnelshift_l(v, v, 8 * TABLE);
+}
+template <typename RkPtr>
+__device__ __forceinline__ void aes128_encrypt(const T0Lane &T, const RkPtr rk, uint32_t (&s)[4]) {
+    uint32_t s0 = s[0] ^ rk[0], s1 = s[1] ^ rk[1], s2 = s[2] ^ rk[2], s3 = s[3] ^ rk[3];
+#pragma unroll
+    for (int r = 1; r < 10; ++r) {
+        const uint32_t t0 = t0_lookup<0, 0>(T, s0) ^ t0_lookup<1, 1>(T, s1) ^ t0_lookup<2, 2>(T, s2) ^ t0_lookup<3, 3>(T, s3) ^ rk[4 * r + 0];
+        const uint32_t t1 = t0_lookup<0, 0>(T, s1) ^ t0_lookup<1, 1>(T, s2) ^ t0_lookup<2, 2>(T, s3) ^ t0_lookup<3, 3>(T, s0) ^ rk[4 * r + 1];
+        const uint32_t t2 = t0_lookup<0, 0>(T, s2) ^ t0_lookup<1, 1>(T, s3) ^ t0_lookup<2, 2>(T, s0) ^ t0_lookup<3, 3>(T, s1) ^ rk[4 * r + 2];
+        const uint32_t t3 = t0_lookup<0, 0>(T, s3) ^ t0_lookup<1, 1>(T, s0) ^ t0_lookup<2, 2>(T, s1) ^ t0_lookup<3, 3>(T, s2) ^ rk[4 * r + 3];
+        s0 = t0; s1 = t1; s2 = t2; s3 = t3;
+    }
+    // final round: SubBytes + ShiftRows; T0 = (2S, S, S, 3S): S is byte 1 (and 2) of every T0 word
+#define FEDS_LAST(a, b, c, d)                                                                                          \
+    __byte_perm(__byte_perm(t0_lookup<0, 0>(T, a), t0_lookup<1, 0>(T, b), 0x3251), __byte_perm(t0_lookup<2, 0>(T, c), t0_lookup<3, 0>(T, d), 0x5210), 0x7610)
+    const uint32_t u0 = FEDS_LAST(s0, s1, s2, s3), u1 = FEDS_LAST(s1, s2, s3, s0), u2 = FEDS_LAST(s2, s3, s0, s1), u3 = FEDS_LAST(s3, s0, s1, s2);
+#undef FEDS_LAST
+    s[0] = u0 ^ rk[40]; s[1] = u1 ^ rk[41]; s[2] = u2 ^ rk[42]; s[3] = u3 ^ rk[43];
+}
 __device__ __forceinline__ void load_t0_replicated(uint32_t *sTab) {
     const uint32_t *src = &g_aes.T[0][0];
     for (int i = threadIdx.x; i < T0_WORDS; i += blockDim.x) sTab[i] = src[i / T0_REPL];
@@ -132,7 +157,8 @@ __global__ void __launch_bounds__(TileShape<C>::CTA, 1) fragment_dct_tile_kernel
     extern __shared__ __align__(16) uint32_t smem[];
     load_t0_replicated(smem);
     T0Lane sT;
-    sT.b = smem + (threadIdx.x & 31);
+    sT.tab = reinterpret_cast<const char *>(smem);
+    sT.lane4 = 4u * (threadIdx.x & 31);
     constexpr ZigzagTable ZZ = make_zigzag();
     const int k = p.k, P = k + 1, Q = 63 - k;
     const int RSQ = tile_run_stride(TB * Q), RSP = tile_run_stride(TB * P);
@@ -198,7 +224,8 @@ __global__ void __launch_bounds__(TileShape<C>::CTA, 1) defragment_dct_tile_kern
     extern __shared__ __align__(16) uint32_t smem[];
     load_t0_replicated(smem);
     T0Lane sT;
-    sT.b = smem + (threadIdx.x & 31);
+    sT.tab = reinterpret_cast<const char *>(smem);
+    sT.lane4 = 4u * (threadIdx.x & 31);
     constexpr ZigzagTable ZZ = make_zigzag();
     const int k = p.k, P = k + 1, Q = 63 - k;
     const int RSQ = tile_run_stride(TB * Q), RSP = tile_run_stride(TB * P);
