@@ -512,7 +512,7 @@ def main():
     # ---------------------------------------------------------------- end to end through the host-buffer C ABI
     e2e = None
     if kind == "dct" and not args.no_e2e:
-        ipc, ns = min(8, n), 4
+        ipc, ns = min(8, n), 8
         streams = [torch.cuda.Stream(device=dev) for _ in range(ns)]
         h_imgs = torch.empty(n * img_bytes, dtype=torch.uint8).pin_memory()
         h_imgs.copy_(d_imgs.view(-1).cpu())
@@ -526,8 +526,18 @@ def main():
                               dtype=torch.uint8, device=dev)
 
         def e2e_step():
-            B.fragment_dct_host(h_imgs, w, h, c, kl, key, h_non, h_priv, h_pub, h_dg, ipc, scratch, streams)
-            B.defragment_dct_host(h_priv, h_pub, n, w, h, c, kl, key, h_non, h_dg, h_out, h_fl, ipc, scratch, streams)
+            # the two host-staged calls, sub-batch by sub-batch (one chunk per stream per call) and with no synchronisation in
+            # between: the fragments of sub-batch i travel to the host while those of sub-batch i-1 travel back, so both PCIe
+            # directions stay busy (the calls share the chunk -> stream mapping, include/feds.h)
+            sub = ipc * ns
+            for a in range(0, n, sub):
+                m = min(sub, n - a)
+                B.fragment_dct_host(h_imgs[a * img_bytes:(a + m) * img_bytes], w, h, c, kl, key, h_non[a:a + m],
+                                    h_priv[a * batch.priv_bytes:(a + m) * batch.priv_bytes], h_pub[a * batch.pub_bytes:(a + m) * batch.pub_bytes],
+                                    h_dg[64 * a:64 * (a + m)], ipc, scratch, streams)
+                B.defragment_dct_host(h_priv[a * batch.priv_bytes:(a + m) * batch.priv_bytes], h_pub[a * batch.pub_bytes:(a + m) * batch.pub_bytes],
+                                      m, w, h, c, kl, key, h_non[a:a + m], h_dg[64 * a:64 * (a + m)], h_out[a * img_bytes:(a + m) * img_bytes],
+                                      h_fl[a:a + m], ipc, scratch, streams)
 
         e2e_step()
         torch.cuda.synchronize()

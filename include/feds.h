@@ -140,8 +140,9 @@ feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w,
 /*
  * Host-staged batch defragment: the mirror image (H2D fragments + nonces [+ expected digests] -> defragment -> D2H
  * images [+ verify flags]). h_expected_digests may be NULL (no verification; h_verify_flags untouched).
- * Uses the same chunk -> stream mapping as feds_fragment_dct_host, so the two may be enqueued back to back on the same
- * streams without a synchronisation in between.
+ * Uses the same chunk -> stream mapping and the same scratch slot per stream as feds_fragment_dct_host (the two scratch
+ * sizes are equal), so the two may be enqueued back to back -- or alternately, sub-batch by sub-batch, which keeps both PCIe
+ * directions busy -- on the same streams and scratch without a synchronisation in between.
  */
 size_t feds_defragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k);
 feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_public, int n_images, int w, int h, int c, int k,

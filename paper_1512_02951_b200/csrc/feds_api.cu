@@ -656,7 +656,9 @@ static size_t host_slot_bytes(int ipc, int w, int h, int c, int k) {
     const size_t pv = round_up((size_t)ipc * feds_dct_private_bytes(w, h, c, k), 256);
     const size_t pb = round_up((size_t)ipc * feds_dct_public_bytes(w, h, c, k), 256);
     const size_t dg = round_up((size_t)ipc * 64, 256), wsb = round_up((size_t)ipc * feds_workspace_bytes(w, h, c, k, 0), 256);
-    return img + non + pv + pb + dg + wsb;
+    // + the verify flags of the defragment call: ONE slot size for both directions, so that stream j owns the same scratch
+    // bytes in either call and the two may be interleaved on the same streams without synchronisation
+    return img + non + pv + pb + dg + wsb + round_up((size_t)ipc * 4, 256);
 }
 
 size_t feds_fragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k) {
@@ -705,7 +707,7 @@ feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w,
 
 size_t feds_defragment_dct_host_scratch_bytes(int images_per_chunk, int n_streams, int w, int h, int c, int k) {
     if (images_per_chunk < 1 || n_streams < 1 || check_dct_args(1, w, h, c, k) != FEDS_OK) return 0;
-    return (host_slot_bytes(images_per_chunk, w, h, c, k) + round_up((size_t)images_per_chunk * 4, 256)) * (size_t)n_streams;
+    return host_slot_bytes(images_per_chunk, w, h, c, k) * (size_t)n_streams;
 }
 
 feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_public, int n_images, int w, int h, int c, int k,
@@ -721,7 +723,7 @@ feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_
         return FEDS_ERR_NULL_POINTER;
     if (misaligned(d_scratch)) return FEDS_ERR_MISALIGNED;
     const int ipc = images_per_chunk;
-    const size_t slot = host_slot_bytes(ipc, w, h, c, k) + round_up((size_t)ipc * 4, 256);
+    const size_t slot = host_slot_bytes(ipc, w, h, c, k);
     if (scratch_bytes < slot * (size_t)n_streams) return FEDS_ERR_WORKSPACE_TOO_SMALL;
     const size_t ws_b = feds_workspace_bytes(w, h, c, k, 0);
     int chunk = 0;
