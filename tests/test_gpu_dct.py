@@ -196,6 +196,42 @@ def test_host_staged_entry_point(orc, b):
         assert (dg.cpu() == h_dg[64 * i:64 * i + 64]).all()
 
 
+def test_host_staged_calls_interleaved_without_sync(orc, b):
+    """fragment and verified defragment of sub-batches alternately on the same streams and the same scratch, no
+    synchronisation until the end (bench.py's e2e pattern): both calls must see the same scratch slot per stream."""
+    n, w, h, c, k = 26, 264, 48, 3, 3
+    ipc, ns = 2, 3
+    key, nonce = synth.key_nonce(41)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=300 + i) for i in range(n)])
+    ib, pb_, qb_ = w * h * c, b.dct_private_bytes(w, h, c, k), b.dct_public_bytes(w, h, c, k)
+    h_imgs = torch.from_numpy(imgs).view(-1).pin_memory()
+    h_non = torch.from_numpy(nonces).pin_memory()
+    h_priv = torch.zeros(n * pb_, dtype=torch.uint8).pin_memory()
+    h_pub = torch.zeros(n * qb_, dtype=torch.uint8).pin_memory()
+    h_dg = torch.zeros(n * 64, dtype=torch.uint8).pin_memory()
+    h_out = torch.zeros(n * ib, dtype=torch.uint8).pin_memory()
+    h_fl = torch.full((n,), 7, dtype=torch.int32).pin_memory()
+    assert b.host_scratch_bytes(ipc, ns, w, h, c, k) == b.defrag_host_scratch_bytes(ipc, ns, w, h, c, k)
+    scratch = torch.empty(b.host_scratch_bytes(ipc, ns, w, h, c, k), dtype=torch.uint8, device="cuda")
+    streams = [torch.cuda.Stream() for _ in range(ns)]
+    sub = ipc * ns
+    for a in range(0, n, sub):
+        m = min(sub, n - a)
+        b.fragment_dct_host(h_imgs[a * ib:(a + m) * ib], w, h, c, k, key, h_non[a:a + m], h_priv[a * pb_:(a + m) * pb_],
+                            h_pub[a * qb_:(a + m) * qb_], h_dg[64 * a:64 * (a + m)], ipc, scratch, streams)
+        b.defragment_dct_host(h_priv[a * pb_:(a + m) * pb_], h_pub[a * qb_:(a + m) * qb_], m, w, h, c, k, key, h_non[a:a + m],
+                              h_dg[64 * a:64 * (a + m)], h_out[a * ib:(a + m) * ib], h_fl[a:a + m], ipc, scratch, streams)
+    for s in streams:
+        s.synchronize()
+    assert torch.equal(h_out, h_imgs) and int(h_fl.abs().sum().item()) == 0
+    # fragments on the host are the ones the device-resident call produces
+    for i in [0, 5, 13, 25]:
+        pv, pu, dg = b.fragment_dct(torch.from_numpy(imgs[i]).cuda(), k, key, nonces[i].tobytes())
+        assert (pv.cpu() == h_priv[i * pb_:(i + 1) * pb_]).all() and (pu.cpu() == h_pub[i * qb_:(i + 1) * qb_]).all()
+        assert (dg.cpu() == h_dg[64 * i:64 * i + 64]).all()
+
+
 # ---------------------------------------------------------------- full BASELINE sizes, in the configuration bench.py times
 def test_config2_full_size(orc, b):
     """4096x4096 RGB, k=5: whole-image stage (ii) + round trip; coefficients on sampled crops (the double DCT is slow)."""
