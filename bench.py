@@ -139,14 +139,14 @@ def run_oracle_jobs(kind, jobs, kl, threads):
     return time.perf_counter() - t0, total
 
 
-def cpu_baseline_sample(kind, w, h, c, kl, target_s=12.0):
+def cpu_baseline_sample(kind, w, h, c, kl, target_s=15.0):
     """The oracle as it stands on a bounded sample: one strip per host thread, passed over repeatedly until about
     `target_s` seconds of wall time have gone by (first pass sizes the repeat count)."""
     threads = min(os.cpu_count() or 1, 16)
     rows = min(120 if kind == "dct" else 256, h)
     jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
     dt1, nbytes1 = run_oracle_jobs(kind, jobs, kl, threads)
-    passes = max(1, min(200, int(target_s / max(dt1, 1e-3))))
+    passes = max(1, min(400, int(round(target_s / max(dt1, 1e-3)))))
     dt, nbytes = run_oracle_jobs(kind, jobs * passes, kl, threads)
     return {"value": nbytes / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": "%d passes over %d strips of %dx%dx%d (one strip per thread), fragment + verified defragment, %.1f s wall"
