@@ -96,6 +96,24 @@ __device__ __forceinline__ void vec_load_global(const uint32_t *src, uint32_t (&
 
 template <typename T, bool GLOBAL>
 __device__ __forceinline__ T ld_ro(const T *q) { return GLOBAL ? __ldg(q) : *q; }
+// uint8 -> float32, exact: byte `pos` of `word` becomes the low mantissa byte of 2^23 (one PRMT), minus 2^23 (one FADD on the
+// FMA pipe) -- instead of shift, mask and I2F on the ALU pipe.
+__device__ __forceinline__ float byte_to_float(uint32_t word, int pos) {
+    return __uint_as_float(__byte_perm(word, 0x4B000000u, 0x7540 + pos)) - 8388608.0f;
+}
+// four float32 -> four uint8 packed little-endian: round to nearest even, saturate to [0,255] (A5). ptxas fuses each
+// pair of conversions with its cvt.pack into one F2IP.U8.F32: two instructions for four pixels.
+__device__ __forceinline__ uint32_t pack4_u8(float a, float b, float c, float d) {
+    int ia, ib, ic, id;
+    asm("cvt.rni.s32.f32 %0, %1;" : "=r"(ia) : "f"(a));
+    asm("cvt.rni.s32.f32 %0, %1;" : "=r"(ib) : "f"(b));
+    asm("cvt.rni.s32.f32 %0, %1;" : "=r"(ic) : "f"(c));
+    asm("cvt.rni.s32.f32 %0, %1;" : "=r"(id) : "f"(d));
+    uint32_t hi, r;
+    asm("cvt.pack.sat.u8.s32.b32 %0, %1, %2, %3;" : "=r"(hi) : "r"(id), "r"(ic), "r"(0));
+    asm("cvt.pack.sat.u8.s32.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(ib), "r"(ia), "r"(hi));
+    return r;
+}
 // GLOBAL = false: `img` is a tile of pixel rows staged in shared memory (same interleaved layout, pitch w pixels)
 template <int C, bool GLOBAL = true>
 __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int w, int y0, int x0, int c, float (&v)[64]) {
@@ -106,8 +124,8 @@ __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int 
             const uint2 q = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row));
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                v[8 * r + i] = (float)((q.x >> (8 * i)) & 0xffu);
-                v[8 * r + 4 + i] = (float)((q.y >> (8 * i)) & 0xffu);
+                v[8 * r + i] = byte_to_float(q.x, i);
+                v[8 * r + 4 + i] = byte_to_float(q.y, i);
             }
         } else if (C == 3) {
             const uint2 q0 = ld_ro<uint2, GLOBAL>(reinterpret_cast<const uint2 *>(row));
@@ -119,14 +137,13 @@ __device__ __forceinline__ void load_block(const uint8_t *__restrict__ img, int 
 #pragma unroll
             for (int j = 0; j < 6; ++j) ws[j] = __funnelshift_r(wd[j], wd[j + 1], 8 * c);
 #pragma unroll
-            for (int i = 0; i < 8; ++i) v[8 * r + i] = (float)((ws[(3 * i) >> 2] >> (8 * ((3 * i) & 3))) & 0xffu);
+            for (int i = 0; i < 8; ++i) v[8 * r + i] = byte_to_float(ws[(3 * i) >> 2], (3 * i) & 3);
         } else {
             const uint4 a = ld_ro<uint4, GLOBAL>(reinterpret_cast<const uint4 *>(row));
             const uint4 b = ld_ro<uint4, GLOBAL>(reinterpret_cast<const uint4 *>(row) + 1);
             const uint32_t wd[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-            const int sh = 8 * c;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) v[8 * r + i] = (float)((wd[i] >> sh) & 0xffu);
+            for (int i = 0; i < 8; ++i) v[8 * r + i] = __uint_as_float(__byte_perm(wd[i], 0x4B000000u, 0x7540u + (uint32_t)c)) - 8388608.0f;
         }
     }
 }
@@ -148,15 +165,8 @@ __device__ __forceinline__ void store_block(uint8_t *__restrict__ img, int w, in
     }
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
-        uint32_t px[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            int q = __float2int_rn(v[8 * r + i]);
-            q = min(max(q, 0), 255);
-            px[i] = (uint32_t)q;
-        }
-        const uint32_t lo = px[0] | (px[1] << 8) | (px[2] << 16) | (px[3] << 24);
-        const uint32_t hi = px[4] | (px[5] << 8) | (px[6] << 16) | (px[7] << 24);
+        const uint32_t lo = pack4_u8(v[8 * r], v[8 * r + 1], v[8 * r + 2], v[8 * r + 3]);
+        const uint32_t hi = pack4_u8(v[8 * r + 4], v[8 * r + 5], v[8 * r + 6], v[8 * r + 7]);
         uint8_t *row = img + ((size_t)(y0 + r) * w + x0) * C;  // start of the strip's 8*C-byte row segment
         if (C == 1) {
             if (act) *reinterpret_cast<uint2 *>(row) = make_uint2(lo, hi);
@@ -183,7 +193,7 @@ __device__ __forceinline__ void store_block(uint8_t *__restrict__ img, int w, in
                 }
             } else if (act) {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) row[i * 3 + c] = (uint8_t)px[i];
+                for (int i = 0; i < 8; ++i) row[i * 3 + c] = (uint8_t)((i < 4 ? lo : hi) >> (8 * (i & 3)));
             }
         } else {
             const uint32_t glo = __shfl_down_sync(0xffffffffu, lo, 1), ghi = __shfl_down_sync(0xffffffffu, hi, 1);
@@ -203,7 +213,7 @@ __device__ __forceinline__ void store_block(uint8_t *__restrict__ img, int w, in
                 }
             } else if (act) {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) row[i * 4 + c] = (uint8_t)px[i];
+                for (int i = 0; i < 8; ++i) row[i * 4 + c] = (uint8_t)((i < 4 ? lo : hi) >> (8 * (i & 3)));
             }
         }
     }
