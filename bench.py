@@ -184,11 +184,14 @@ def reference_arm(args, kind, n, w, h, c, kl, desc):
 def sweep_arm(args, desc):
     """BASELINE configs[4]: fragment + verified defragment per point, device-resident, CUDA events; MB/s of image and the
     algorithmic HBM GB/s (DCT: 5 B per pixel-channel and direction; DWT: 3 B) against the measured copy rate."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return   # the sweep is a single-GPU table: under torchrun rank 0 alone runs it
     import torch
     import synth
     from paper_1512_02951_b200 import binding as B
-    torch.cuda.set_device(0)
-    dev = torch.device("cuda", 0)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
     hbm_peak, _, peak_src = peaks()
     key, nonce = synth.key_nonce(5)
     points = []
