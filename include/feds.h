@@ -43,7 +43,8 @@ typedef enum {
 
 /* Flags for the *_batch entry points. */
 #define FEDS_FLAG_NONE 0u
-#define FEDS_FLAG_NO_DIGEST 1u /* skip step 5 (SHA-256 Merkle digests); d_digests is not written. Measurement of the HBM-bound core. */
+#define FEDS_FLAG_NO_DIGEST 1u /* skip step 5 (SHA-256 Merkle digests): the report's own selective encryption (DCT + select + AES,
+                                  P:488-494), HBM-bound. d_digests is not written; defragment does not verify. */
 
 const char *feds_status_string(feds_status s);
 int feds_last_cuda_error(void); /* cudaError_t of the most recent FEDS_ERR_CUDA on this thread, else 0 */
