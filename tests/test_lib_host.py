@@ -123,3 +123,17 @@ def test_device_zigzag_table(b, paper_pins):
     assert sorted(out) == list(range(64))
     for a, c in zip(zz, zz[1:]):
         assert max(abs(a[0] - c[0]), abs(a[1] - c[1])) == 1
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/feds.h is a C ABI: it must compile as C99 with nothing but the standard headers (no CUDA, no C++)."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "use_feds.c"
+    src.write_text('#include "feds.h"\nint main(void) { feds_stream_t s = 0; (void)s; return (int)feds_dct_private_bytes(8, 8, 1, 0) == 4 ? 0 : 1; }\n')
+    res = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), str(src)],
+                         capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
