@@ -145,8 +145,9 @@ def cpu_baseline_sample(kind, w, h, c, kl, target_s=15.0):
     threads = min(os.cpu_count() or 1, 16)
     rows = min(120 if kind == "dct" else 256, h)
     jobs = oracle_sample_jobs(kind, w, h, c, kl, threads, seed=9000)
-    dt1, nbytes1 = run_oracle_jobs(kind, jobs, kl, threads)
-    passes = max(1, min(400, int(round(target_s / max(dt1, 1e-3)))))
+    run_oracle_jobs(kind, jobs, kl, threads)                     # loads the library, starts the pool: not representative
+    dt1, nbytes1 = run_oracle_jobs(kind, jobs, kl, threads)      # one warm pass sizes the sample
+    passes = max(1, min(1000, int(round(target_s / max(dt1, 1e-3)))))
     dt, nbytes = run_oracle_jobs(kind, jobs * passes, kl, threads)
     return {"value": nbytes / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": "%d passes over %d strips of %dx%dx%d (one strip per thread), fragment + verified defragment, %.1f s wall"
