@@ -315,7 +315,7 @@ def main():
         batch = B.DctBatch(n, w, h, c, kl, device=dev)
         nl = c * (h // 8) * ((w // 8 + 7) // 8)
         tree_launches = tree_launch_count(nl)
-        per_step_launches = (1 + tree_launches) + (1 + tree_launches + 1)
+        per_step_launches = (1 + tree_launches) + (2 + tree_launches + 1)   # fragment + tree | leaf hash + reconstruction + tree + compare
 
         def step(record=False):
             if record:

@@ -90,6 +90,21 @@ feds_status feds_defragment_dct(const uint8_t *d_private, const uint8_t *d_publi
                                 size_t workspace_bytes, feds_stream_t stream);
 
 /*
+ * feds_verify_dct — the integrity half of step 6 alone ("integrity requirement"; A8, A10): recomputes the
+ * Merkle roots of the two fragments as they lie in memory and compares them with d_expected_digests (64 bytes per image).
+ * Needs no key: the digests cover the stored bytes (ciphertext / plaintext coefficients), so whoever holds a fragment
+ * can check it. d_verify_flags[i] = bit0 (private mismatch) | bit1 (public mismatch). Workspace as for feds_defragment_dct.
+ * feds_verify_dct_batch: n_images fragments at the given byte strides (as feds_defragment_dct_batch).
+ */
+feds_status feds_verify_dct(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k,
+                            const uint8_t *d_expected_digests, uint32_t *d_verify_flags, void *d_workspace,
+                            size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_verify_dct_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public,
+                                  size_t public_stride, int n_images, int w, int h, int c, int k,
+                                  const uint8_t *d_expected_digests, uint32_t *d_verify_flags, void *d_workspace,
+                                  size_t workspace_bytes, feds_stream_t stream);
+
+/*
  * feds_fragment_dwt / feds_defragment_dwt — rows D1-D8: level shift -128, `levels`-level whole-image
  * Le Gall 5/3 integer lifting, rows then columns, LL_levels -> private under AES-128-CTR,
  * the other subbands -> public (order: channel, level L..1, HL, LH, HH, row-major int16 LE), SHA-256 Merkle
@@ -176,8 +191,9 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
 
 /*
  * Profiling hook (not part of the data path; thread-local): while set, every fragment/defragment call made on this
- * thread records ev_start immediately before and ev_stop immediately after its dominant kernel, on the call's stream:
- * the fused tile kernel of the DCT path, the leaf-hashing kernel of the DWT path.
+ * thread records ev_start immediately before and ev_stop immediately after its dominant kernel(s), on the call's stream:
+ * DCT fragment: the fused kernel; DCT verified defragment: the leaf-hash kernel and the reconstruction kernel together;
+ * digest-free DCT calls: the tile kernel; feds_verify_dct: the leaf-hash kernel; DWT path: the leaf-hashing kernel.
  * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.
  */
 void feds_profile_events(void *ev_start, void *ev_stop);

@@ -26,7 +26,7 @@ SYMBOLS = [
     "feds_fragment_dct_batch", "feds_defragment_dct_batch",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
-    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle",
+    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
 ]
 
@@ -63,6 +63,8 @@ def _load():
     lib.feds_defragment_dct_host_scratch_bytes.restype = sz
     lib.feds_defragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_defragment_dct_host.argtypes = [vp, vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
+    lib.feds_verify_dct.argtypes = [vp, vp, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.feds_verify_dct_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.feds_aes128_ctr.argtypes = [vp, vp, sz, u8p, u8p, vp]
     lib.feds_sha256_merkle_workspace_bytes.restype = sz
     lib.feds_sha256_merkle_workspace_bytes.argtypes = [sz]
@@ -75,7 +77,7 @@ def _load():
     lib.feds_debug_zigzag_host.argtypes = [vp]
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
                  "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host",
-                 "feds_aes128_ctr", "feds_sha256_merkle"]:
+                 "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch"]:
         getattr(lib, name).restype = i
     return lib
 
@@ -159,6 +161,16 @@ def defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=None, stream=None
     return out, flags
 
 
+def verify_dct(priv, pub, w, h, c, k, expected, stream=None, workspace=None):
+    """feds_verify_dct: integrity of the two fragments against their 64-byte digest pair, no key needed -> flags tensor [1]."""
+    dev = priv.device
+    flags = torch.zeros(1, dtype=torch.int32, device=dev)
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _check(lib.feds_verify_dct(_ptr(priv), _ptr(pub), w, h, c, k, _ptr(expected), _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)),
+           "feds_verify_dct")
+    return flags
+
+
 def fragment_dwt(image, levels, key, nonce, stream=None, workspace=None):
     image, w, h, c = _hwc(image)
     dev = image.device
@@ -227,6 +239,15 @@ class DctBatch:
                                              self.c, self.k, bytes(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
                                              self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
                                              _stream(stream)), "feds_defragment_dct_batch")
+
+
+    def verify(self, expected=None, stream=None):
+        """feds_verify_dct_batch on the batch's own fragments (expected defaults to its own digests) -> flags_out."""
+        expected = self.digests if expected is None else expected
+        _check(lib.feds_verify_dct_batch(_ptr(self.priv), self.priv_bytes, _ptr(self.pub), self.pub_bytes, self.n, self.w, self.h, self.c,
+                                         self.k, _ptr(expected), _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), _stream(stream)),
+               "feds_verify_dct_batch")
+        return self.flags_out
 
 
 def fragment_dct_host(h_images, w, h, c, k, key, h_nonces, h_priv, h_pub, h_digests, images_per_chunk, d_scratch, streams,

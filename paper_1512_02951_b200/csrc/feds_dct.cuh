@@ -1,4 +1,5 @@
-// feds_dct.cuh — fused DCT-path kernels, sm_100a.
+// feds_dct.cuh — the fused fragment kernel of the DCT path and the block load / store /
+// slot helpers the other DCT kernels share (feds_dct_tile.cuh: digest-free kernels, leaf-hash kernel), sm_100a.
 //
 // One thread owns one Merkle leaf = up to G consecutive 8x8 blocks of one block row of one channel
 // (DESIGN.md 2.1). For each block it: loads the 8x8 pixels, runs the separable FP32 DCT in 64 registers,
@@ -27,10 +28,6 @@ __device__ const AesTables g_aes = make_aes_tables();
 constexpr int DCT_THREADS = FEDS_FRAG_THREADS;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
 constexpr int DCT_CTAS_PER_SM = 1;
 constexpr size_t DCT_SMEM_MAX = 227 * 1024;
-#ifndef FEDS_DEFRAG_THREADS
-#define FEDS_DEFRAG_THREADS 384
-#endif
-constexpr int DEFRAG_THREADS = FEDS_DEFRAG_THREADS;
 constexpr int AES_TABLE_WORDS = 1024;
 constexpr int CA = 16;  // carry area: a SHA-256 block is 16 words, at most 15 (16 - V) words wait between blocks
 
@@ -545,114 +542,6 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
         store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
     }
     if (V == 1) __syncwarp();  // the next group's first copy-out reads every lane's slot
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// defragment: steps 6-8 (+ recomputation of the leaf digests of the fragments as received when VERIFY)
-// ------------------------------------------------------------------------------------------------------------
-template <int C, int V, bool VERIFY>
-__global__ void __launch_bounds__(DEFRAG_THREADS, DCT_CTAS_PER_SM) defragment_dct_kernel(const __grid_constant__ DctParams p) {
-    extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *sT = smem;
-    load_aes_tables(sT);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *wslots = smem + AES_TABLE_WORDS + warp * 32 * p.slot_stride;
-    uint32_t *my = wslots + lane * p.slot_stride;
-    constexpr ZigzagTable ZZ = make_zigzag();
-
-    const int k = p.k, P = k + 1, Q = 63 - k;
-    uint32_t *mp = my + CA;
-    uint32_t *mq = my + 2 * CA;
-#pragma unroll 1
-    for (unsigned grp = (unsigned)warp * gridDim.x + blockIdx.x; grp < p.n_groups; grp += (blockDim.x >> 5) * gridDim.x) {
-    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)grp * 32 + lane);
-    uint8_t *img = p.images_out + (size_t)L.n * p.image_stride;
-    const uint32_t *pub_src = reinterpret_cast<const uint32_t *>(p.pub + (size_t)L.n * p.pub_stride) + (size_t)L.b0 * Q;
-    const uint32_t *priv_src = reinterpret_cast<const uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
-    uint32_t nonce[4];
-    load_nonce(p, L.n, nonce);
-
-    ShaStream cur;
-    ShaMeta oth;
-    const int hoff = dct_stash_offset(k);
-    sha256_init(cur.H);
-    if (VERIFY) stash_init<V>(my, hoff);
-    cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
-    oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
-    Keystream K;
-    K.blk = ~0ull;
-    const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
-
-#pragma unroll 1
-    for (int s = 0; s <= G_BLOCKS; ++s) {
-        const bool act = s < L.nblk;
-        const uint32_t *pq = pub_src + (size_t)s * Q - P;  // indexed by z
-        const uint32_t *pv = priv_src + (size_t)s * P;
-        if (s < G_BLOCKS) {
-            if (V == 1) {
-                warp_copy_runs<false>(wslots, p.slot_stride, P, Q, act ? reinterpret_cast<unsigned long long>(pq + P) : 0ull,
-                                      act ? reinterpret_cast<unsigned long long>(pv) : 0ull);
-                __syncwarp();
-            } else if (act) {
-                // each lane pulls its own runs: all loads first, then the stores into the slot
-#pragma unroll
-                for (int g0 = 0; g0 < 64; g0 += 8 * V) {
-                    uint32_t x[8][V];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int g = g0 + i * V;
-                        if (g < P) vec_load_global<V>(pv + g, x[i]); else vec_load_global<V>(pq + g, x[i]);
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const int g = g0 + i * V;
-                        vec_store<V>(g < P ? mp + g : mq + g, x[i]);
-                    }
-                }
-            }
-            if (VERIFY) { cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0; }
-        }
-        if (VERIFY) {
-#pragma unroll 1
-            for (int it = 0; it < 2; ++it) {
-                if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb<V>(my, cur, p.one);  // hashes the bytes as received; leaves [base+16, ..) of the current block intact
-                swap_streams<V>(my, hoff, cur, oth);
-            }
-        }
-        if (s < G_BLOCKS) {
-            float v[64];
-            if (act) {
-                const unsigned long long w0 = priv_word0 + (unsigned long long)s * P;
-#pragma unroll 1
-                for (int j = 0; j < P; j += V) {
-                    uint32_t ks[V], x[V];
-                    keystream_words<V>(K, sT, p.rk, nonce, w0 + j, ks);
-                    vec_load<V>(mp + j, x);
-#pragma unroll
-                    for (int t = 0; t < V; ++t) x[t] ^= ks[t];
-                    vec_store<V>(mp + j, x);
-                }
-#pragma unroll
-                for (int g = 0; g < 64; g += V) {
-                    uint32_t x[V];
-                    vec_load<V>(g < P ? mp + g : mq + g, x);
-#pragma unroll
-                    for (int t = 0; t < V; ++t) v[ZZ.pos[g + t]] = __uint_as_float(x[t]);
-                }
-                idct8x8(v);
-            }
-            store_block<C>(img, p.w, 8 * L.br, 8 * (L.g * G_BLOCKS + s), L.c, act, v);
-            if (V == 1) __syncwarp();  // the next phase's copy-in overwrites the slots
-        }
-    }
-    if (VERIFY && L.valid) {
-        const size_t nl = p.leaves_per_image;
-        if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
-        stash_read<V>(my, hoff, cur.H);  // after an even number of swaps the private stream is the stashed one
-        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
-    }
     }
 }
 

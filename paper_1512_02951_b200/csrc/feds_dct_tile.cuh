@@ -282,4 +282,66 @@ __global__ void __launch_bounds__(TileShape<C>::CTA, 1) defragment_dct_tile_kern
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Leaf digests of DCT fragments as they lie in memory, nothing else (the verification half of steps 6-8, and
+// all of feds_verify_dct): one thread per (fragment, leaf), registers only, 28 warps per SM. A leaf's bytes are contiguous in its fragment (G consecutive blocks of one block row), so this is SHA-256
+// of a word-aligned byte range; needs no key. Threads [0, total_leaves) take the public leaves (31 compressions at k = 3),
+// the rest the private ones (3 compressions), so that the lanes of a warp walk chains of equal length.
+// ------------------------------------------------------------------------------------------------------------
+constexpr int LEAFHASH_THREADS = 128;
+template <int C>
+__global__ void __launch_bounds__(LEAFHASH_THREADS) dct_leaves_hash_kernel(const __grid_constant__ DctParams p) {
+    const unsigned long long gid = (unsigned long long)blockIdx.x * LEAFHASH_THREADS + threadIdx.x;
+    if (gid >= 2 * p.total_leaves) return;
+    const bool priv = gid >= p.total_leaves;
+    const LeafCoord L = decode_leaf<C>(p, priv ? gid - p.total_leaves : gid);
+    const int W = priv ? p.k + 1 : 63 - p.k;   // words per block in this fragment
+    if (W == 0) return;                        // k = 63: the public fragment is empty, its root is written elsewhere
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(priv ? p.priv + (size_t)L.n * p.priv_stride : p.pub + (size_t)L.n * p.pub_stride) +
+                          (size_t)L.b0 * W;
+    const unsigned nwords = (unsigned)(L.nblk * W);
+    const bool al16 = (reinterpret_cast<uintptr_t>(src) & 15u) == 0;
+    uint32_t H[8], w[16], nx[16];
+    sha256_init(H);
+    const unsigned full = nwords >> 4, tail = nwords & 15u;
+    auto fetch = [&](unsigned blk) {
+        const uint32_t *q = src + 16 * (size_t)blk;
+        if (al16) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const uint4 v = __ldg(reinterpret_cast<const uint4 *>(q) + i);
+                nx[4 * i] = v.x; nx[4 * i + 1] = v.y; nx[4 * i + 2] = v.z; nx[4 * i + 3] = v.w;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) nx[i] = __ldg(q + i);
+        }
+    };
+    if (full > 0) fetch(0);
+#pragma unroll 1
+    for (unsigned i = 0; i < full; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) w[j] = bswap32(nx[j]);
+        if (i + 1 < full) fetch(i + 1);
+        sha256_compress_rolled_fma(H, w, p.one);
+    }
+    // tail words, the 0x80 marker and the bit length (FIPS 180-4 5.1.1); one more block when fewer than 3 words are free
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        uint32_t x = 0u;
+        if ((unsigned)j < tail) x = bswap32(__ldg(src + 16 * (size_t)full + j));
+        else if ((unsigned)j == tail) x = 0x80000000u;
+        w[j] = x;
+    }
+    const unsigned long long bits = (unsigned long long)nwords * 32ull;
+    if (tail > 13u) {
+        sha256_compress_rolled_fma(H, w, p.one);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) w[j] = 0u;
+    }
+    w[14] = (uint32_t)(bits >> 32); w[15] = (uint32_t)bits;
+    sha256_compress_rolled_fma(H, w, p.one);
+    store_digest(p.leaves + (((size_t)L.n * 2 + (priv ? 0 : 1)) * p.leaves_per_image + L.li) * 32, H);
+}
+
 }  // namespace feds

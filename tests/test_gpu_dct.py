@@ -130,6 +130,30 @@ def test_verify_flags_and_error_confinement(orc, b):
     assert (bad != d_img).float().mean().item() > 0.5            # wrong key does not reconstruct
 
 
+@pytest.mark.parametrize("w,h,c,k", [(264, 48, 3, 3), (72, 8, 1, 0), (1032, 16, 1, 5), (136, 24, 4, 63), (2048, 16, 3, 9)])
+def test_verify_without_key(orc, b, w, h, c, k):
+    """feds_verify_dct: a fragment holder checks integrity against the digest pair with no key (A8); every single
+    flipped byte of either fragment is confined to its own flag bit."""
+    img = synth.image(w, h, c, seed=w + k)
+    key, nonce = synth.key_nonce(w + 1)
+    priv, pub, dg = b.fragment_dct(torch.from_numpy(img).cuda(), k, key, nonce)
+    # the digests are the oracle's for these stored bytes
+    assert dg.cpu().numpy().tobytes() == orc.fragment_from_coef32(
+        gpu_coefficients(orc, priv.cpu().numpy(), pub.cpu().numpy(), c * (h // 8) * (w // 8), k, key, nonce), w, h, c, k, key, nonce)[2]
+    assert int(b.verify_dct(priv, pub, w, h, c, k, dg).item()) == 0
+    rng = np.random.default_rng(w)
+    for _ in range(4):
+        p2 = priv.clone()
+        p2[int(rng.integers(0, priv.numel()))] ^= 1 << int(rng.integers(0, 8))
+        assert int(b.verify_dct(p2, pub, w, h, c, k, dg).item()) == 1
+        if pub.numel() > 16 and k < 63:
+            q2 = pub.clone()
+            q2[int(rng.integers(0, b.dct_public_bytes(w, h, c, k)))] ^= 1 << int(rng.integers(0, 8))
+            assert int(b.verify_dct(priv, q2, w, h, c, k, dg).item()) == 2
+    d2 = dg.clone(); d2[40] ^= 4
+    assert int(b.verify_dct(priv, pub, w, h, c, k, d2).item()) == 2
+
+
 def test_counter_carry_on_device(orc, b):
     # nonce just below the 32-bit and 64-bit carry boundaries (DESIGN.md A6)
     img = synth.image(64, 32, 1, seed=8)
@@ -165,6 +189,8 @@ def test_batch_equals_singles(orc, b):
     batch.pub[batch.pub_bytes * 3 + 5] ^= 0x80
     batch.defragment(out, key, d_nonces, expected=batch.digests)
     assert batch.flags_out.cpu().tolist() == [0, 0, 0, 2, 0]
+    batch.flags_out.zero_()
+    assert batch.verify().cpu().tolist() == [0, 0, 0, 2, 0]
     # no-digest flag: same fragment bytes, digests untouched
     batch2 = b.DctBatch(n, w, h, c, k)
     batch2.digests.fill_(7)
