@@ -418,9 +418,15 @@ int dwt_fast_px(const DwtLevelParams &p, bool u8, int c_img) {
     if (u8) { if (p.img_w % (c_img == 1 ? 16 : 8)) return 0; }
     return px;
 }
-dim3 dwt_fast_grid(const DwtLevelParams &p, int px, int planes) {
+// picks the rows per warp tile (p.rows) so that the launch has at least ~12 warps per SM, and returns the grid
+dim3 dwt_fast_grid(DwtLevelParams &p, int px, int planes) {
     const int runs = p.cw / px, bh = p.ch >> 1;
-    return dim3((runs + DWTF_LANES_OUT - 1) / DWTF_LANES_OUT, (bh + DWTF_WARPS * DWTF_ROWS - 1) / (DWTF_WARPS * DWTF_ROWS), planes);
+    const unsigned strips = (unsigned)((runs + DWTF_LANES_OUT - 1) / DWTF_LANES_OUT);
+    const unsigned long long want = 12ull * (unsigned)sm_count();
+    int rows = DWTF_ROWS;
+    while (rows > 4 && (unsigned long long)strips * planes * ((bh + rows - 1) / rows) < want) rows /= 2;
+    p.rows = rows;
+    return dim3(strips, (unsigned)((bh + DWTF_WARPS * rows - 1) / (DWTF_WARPS * rows)), planes);
 }
 
 // AES-128-CTR of a byte stream: the conflict-free 128 KB table layout pays once the stream is a few MB long
@@ -603,9 +609,10 @@ feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int l
         p.pub_chan_stride = pl.pub_b / 2 / c;
         p.level_off = dwt_level_off_elems(w, h, L, l);
         const int px = dwt_fast_px(p, l == 1, c);
-        if (px && l == 1 && c == 1) dwt_fwd_fast_kernel<1, 16, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px && l == 1) dwt_fwd_fast_kernel<3, 8, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px) dwt_fwd_fast_kernel<1, 16, false><<<dwt_fast_grid(p, px, c), DWTF_WARPS * 32, 0, stream>>>(p);
+        const dim3 fgrid = px ? dwt_fast_grid(p, px, l == 1 ? 1 : c) : dim3();   // also sets p.rows
+        if (px && l == 1 && c == 1) dwt_fwd_fast_kernel<1, 16, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px && l == 1) dwt_fwd_fast_kernel<3, 8, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px) dwt_fwd_fast_kernel<1, 16, false><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
         else {
             const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
             if (l == 1) dwt_fwd_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
@@ -662,9 +669,10 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
         p.img_out = d_image_out;
         if (l > 1) { p.ll_out_plane = reinterpret_cast<int16_t *>(ws + pl.plane_off[l - 1]); p.ll_out_plane_stride = (size_t)p.cw * p.ch; }
         const int px = dwt_fast_px(p, l == 1, c);
-        if (px && l == 1 && c == 1) dwt_inv_fast_kernel<1, 16, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px && l == 1) dwt_inv_fast_kernel<3, 8, true><<<dwt_fast_grid(p, px, 1), DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px) dwt_inv_fast_kernel<1, 16, false><<<dwt_fast_grid(p, px, c), DWTF_WARPS * 32, 0, stream>>>(p);
+        const dim3 fgrid = px ? dwt_fast_grid(p, px, l == 1 ? 1 : c) : dim3();   // also sets p.rows
+        if (px && l == 1 && c == 1) dwt_inv_fast_kernel<1, 16, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px && l == 1) dwt_inv_fast_kernel<3, 8, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
+        else if (px) dwt_inv_fast_kernel<1, 16, false><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
         else {
             const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
             if (l == 1) dwt_inv_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);

@@ -38,6 +38,7 @@ struct DwtLevelParams {
     int16_t *pub;            // public fragment base; band b (0 HL, 1 LH, 2 HH) of plane (n,c) at
                              // pub + n*pub_image_stride + c*pub_chan_stride + level_off + b*bw*bh (elements)
     size_t pub_image_stride, pub_chan_stride, level_off;
+    int rows;                // streaming kernels (feds_dwt_fast.cuh): subband rows per warp tile
 };
 
 __device__ __forceinline__ bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }

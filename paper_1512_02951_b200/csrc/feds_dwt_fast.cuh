@@ -13,7 +13,8 @@
 namespace feds {
 
 constexpr int DWTF_WARPS = 4;         // warps per CTA, stacked vertically (consecutive row tiles of one column strip)
-constexpr int DWTF_ROWS = 16;         // subband rows per warp tile
+constexpr int DWTF_ROWS = 16;         // subband rows per warp tile on large levels; DwtLevelParams::rows (16, 8 or 4) is what a launch uses:
+                                      // small levels take shorter tiles so that the grid still fills the SMs (each tile re-reads 3 halo rows)
 constexpr int DWTF_LANES_OUT = 30;    // lanes 1..30 write; 0 and 31 are halo
 
 template <int N>
@@ -128,9 +129,9 @@ __global__ void __launch_bounds__(DWTF_WARPS * 32) dwt_fwd_fast_kernel(const __g
     const bool in_range = px0 >= 0 && px0 < p.cw;
     const bool writer = in_range && lane >= 1 && lane <= DWTF_LANES_OUT;
     const bool first_run = px0 == 0, last_run = px0 + PX == p.cw;
-    const int m0 = ((int)blockIdx.y * DWTF_WARPS + warp) * DWTF_ROWS;
+    const int m0 = ((int)blockIdx.y * DWTF_WARPS + warp) * p.rows;
     if (m0 >= bh) return;  // whole warp
-    const int m1 = min(m0 + DWTF_ROWS, bh);
+    const int m1 = min(m0 + p.rows, bh);
     // plane bookkeeping: U8 -> blockIdx.z = image n, all C channels here; else blockIdx.z = plane index n*Cimg + c
     const int n = U8 ? (int)blockIdx.z : (int)blockIdx.z / p.C, c0 = U8 ? 0 : (int)blockIdx.z % p.C;
     const void *base = U8 ? static_cast<const void *>(p.img_in + (size_t)n * p.image_stride)
@@ -248,9 +249,9 @@ __global__ void __launch_bounds__(DWTF_WARPS * 32) dwt_inv_fast_kernel(const __g
     const bool in_range = px0 >= 0 && px0 < p.cw;
     const bool writer = in_range && lane >= 1 && lane <= DWTF_LANES_OUT;
     const bool first_run = px0 == 0, last_run = px0 + PX == p.cw;
-    const int m0 = ((int)blockIdx.y * DWTF_WARPS + warp) * DWTF_ROWS;
+    const int m0 = ((int)blockIdx.y * DWTF_WARPS + warp) * p.rows;
     if (m0 >= bh) return;
-    const int m1 = min(m0 + DWTF_ROWS, bh);
+    const int m1 = min(m0 + p.rows, bh);
     const int n = U8 ? (int)blockIdx.z : (int)blockIdx.z / p.C, c0 = U8 ? 0 : (int)blockIdx.z % p.C;
     void *base = U8 ? static_cast<void *>(p.img_out + (size_t)n * p.image_stride)
                     : static_cast<void *>(p.ll_out_plane + (size_t)blockIdx.z * p.ll_out_plane_stride);
