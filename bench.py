@@ -315,7 +315,11 @@ def main():
         batch = B.DctBatch(n, w, h, c, kl, device=dev)
         nl = c * (h // 8) * ((w // 8 + 7) // 8)
         tree_launches = tree_launch_count(nl)
-        per_step_launches = (1 + tree_launches) + (2 + tree_launches + 1)   # fragment + tree | leaf hash + reconstruction + tree + compare
+        # steps 1-5 run in the fused kernel when its persistent grid is full and k + 1 is even, else as tile kernel + leaf-hash
+        # kernel (the library's rule, feds_api.cu fragment_fused_pays)
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        frag_fused = (kl + 1) % 2 == 0 and (n * nl + 31) // 32 >= 2 * 16 * sms
+        per_step_launches = ((1 if frag_fused else 2) + tree_launches) + (2 + tree_launches + 1)   # | leaf hash + reconstruction + tree + compare
 
         def step(record=False):
             if record:
@@ -413,7 +417,8 @@ def main():
         alu_ops = n * c * (h // 8) * per_row
         alu_peak = 148 * 64 * sm_max_mhz * 1e6 / 1e12  # 148 SMs x 4 SMSPs x 16 ALU-pipe lanes/clk (B300_MICROARCH: rt_SMSP = 2)
         achieved = alu_ops / (frag_ms * 1e-3) / 1e12
-        vname = "fragment_dct_kernel<%d,%d,true>" % (c, 4 if P % 4 == 0 else 2 if P % 2 == 0 else 1)
+        vname = ("fragment_dct_kernel<%d,%d>" % (c, 4 if P % 4 == 0 else 2)) if frag_fused else \
+                ("fragment_dct_tile_kernel<%d,%d> + dct_leaves_hash_kernel<%d>" % (c, 4 if P % 4 == 0 else 2 if P % 2 == 0 else 1, c))
         traffic = None
         tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
         if os.path.exists(tpath):

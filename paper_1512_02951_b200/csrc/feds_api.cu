@@ -230,14 +230,29 @@ feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream) {
     return FEDS_OK;
 }
 
-template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V, true>, p, s); } };
+template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V>, p, s); } };
 template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(fragment_dct_tile_kernel<C, V>, p, s); } };
 template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(defragment_dct_tile_kernel<C, V>, p, s); } };
 template <int C, int V> struct DefragAfterHash { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(defragment_dct_tile_kernel<C, V>, p, s, false); } };
 
-template <bool DIGEST>
-feds_status launch_fragment(const DctParams &p, int c, cudaStream_t stream) {
-    return DIGEST ? dispatch_cv<FragDigest>(p, c, stream) : dispatch_cv<FragPlain>(p, c, stream);
+feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream) { return dispatch_cv<FragPlain>(p, c, stream); }
+// the fused kernel exists for V = 4 and V = 2 only
+feds_status launch_fragment_fused(const DctParams &p, int c, cudaStream_t stream) {
+    const int V = dct_vec_width(p.k);
+#define FEDS_V(CC) (V == 4 ? FragDigest<CC, 4>::go(p, stream) : FragDigest<CC, 2>::go(p, stream))
+    return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
+#undef FEDS_V
+}
+// Steps 1-5 in one fused kernel pay when its persistent grid is full (16 warps per SM for at least two rounds) and the runs
+// are 8- or 16-byte multiples; otherwise the digest-free tile kernel followed by the leaf-hash kernel of what it wrote is
+// faster (measured: 11 % at 512^2, 3 % at one 4096^2 image, 2-4 % for odd k + 1 at any size; 3 % slower at cfg3).
+bool fragment_fused_pays(const DctParams &p) {
+    if (dct_vec_width(p.k) == 1) return false;
+    if (const char *force = getenv("FEDS_FRAGMENT_PATH")) {   // test hook: "fused" | "split"
+        if (force[0] == 'f') return true;
+        if (force[0] == 's') return false;
+    }
+    return p.n_groups >= 2u * (DCT_THREADS / 32) * (unsigned)sm_count();
 }
 feds_status launch_defragment(const DctParams &p, int c, cudaStream_t stream, bool after_hash = false) {
     return after_hash ? dispatch_cv<DefragAfterHash>(p, c, stream) : dispatch_cv<DefragPlain>(p, c, stream);
@@ -269,7 +284,14 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
     uint8_t *ws = static_cast<uint8_t *>(d_workspace);
     p.leaves = (pl.nl > 1) ? ws : d_digests;  // a one-leaf fragment's root is its leaf digest
     if (digest) {
-        st = launch_fragment<true>(p, c, stream);
+        if (fragment_fused_pays(p)) {
+            st = launch_fragment_fused(p, c, stream);
+        } else {
+            st = launch_fragment_tile(p, c, stream);   // records the profiling start; the stop follows the leaf hash
+            if (st != FEDS_OK) return st;
+            st = launch_leaves_hash(p, c, stream);
+            if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
+        }
         if (st != FEDS_OK) return st;
         if (pl.nl > 1) {
             st = run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, d_digests, 32, k == 63 ? 1 : 0, stream);
@@ -280,7 +302,7 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
             FEDS_LAUNCH_CHECK();
         }
     } else {
-        st = launch_fragment<false>(p, c, stream);
+        st = launch_fragment_tile(p, c, stream);
         if (st != FEDS_OK) return st;
     }
     return FEDS_OK;

@@ -13,8 +13,9 @@
 // P = k+1 (then it divides Q = 64-P too, and every run starts 4V-byte aligned):
 //   V = 4 / 2 : each lane moves its own runs with 128 / 64-bit accesses straight from / to registers; no warp
 //               cooperation, no barrier in the block loop.
-//   V = 1     : 4-byte runs would scatter 64 stores per block over 32 lines each, so the warp copies every
-//               lane's runs through the slots with coalesced 32-bit accesses instead.
+//   k + 1 odd : 4-byte runs would scatter 64 stores per block over 32 lines each; the host routes those k to the tile
+//               kernel followed by the leaf-hash kernel (feds_dct_tile.cuh), which measured 2-4 % faster than a
+//               warp-cooperative copy inside this kernel did.
 #pragma once
 #include "feds_device.cuh"
 
@@ -399,57 +400,10 @@ __device__ __forceinline__ void keystream_words(Keystream &K, const Tab sT, cons
     }
 }
 
-// V == 1 only: the warp moves every active lane's public (Q words) and private (P words) run between the lanes' slots
-// and global memory with coalesced 32-bit accesses. pd / vd: this lane's run pointers for the phase (0 = inactive).
-template <bool TO_GLOBAL>
-__device__ __forceinline__ void warp_copy_runs(uint32_t *wslots, int stride, int P, int Q, unsigned long long pd, unsigned long long vd) {
-    const int lane = threadIdx.x & 31;
-#pragma unroll 1
-    for (int l0 = 0; l0 < 32; l0 += 4) {
-        unsigned long long pq[4], vq[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) { pq[i] = __shfl_sync(0xffffffffu, pd, l0 + i); vq[i] = __shfl_sync(0xffffffffu, vd, l0 + i); }
-        if (TO_GLOBAL) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                if (vq[i] == 0ull) continue;
-                const uint32_t *src = wslots + (l0 + i) * stride;
-                uint32_t *dq = reinterpret_cast<uint32_t *>(pq[i]);
-                uint32_t *dp = reinterpret_cast<uint32_t *>(vq[i]);
-                if (lane < Q) dq[lane] = src[2 * CA + P + lane];
-                if (lane + 32 < Q) dq[lane + 32] = src[2 * CA + P + lane + 32];
-                if (lane < P) dp[lane] = src[CA + lane];
-                if (lane + 32 < P) dp[lane + 32] = src[CA + lane + 32];
-            }
-        } else {
-            uint32_t t[4][4];  // all loads of four runs are issued before the first store: one latency, not sixteen
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const bool on = vq[i] != 0ull;
-                const uint32_t *sq = reinterpret_cast<const uint32_t *>(pq[i]);
-                const uint32_t *sp = reinterpret_cast<const uint32_t *>(vq[i]);
-                t[i][0] = (on && lane < Q) ? __ldg(sq + lane) : 0u;
-                t[i][1] = (on && lane + 32 < Q) ? __ldg(sq + lane + 32) : 0u;
-                t[i][2] = (on && lane < P) ? __ldg(sp + lane) : 0u;
-                t[i][3] = (on && lane + 32 < P) ? __ldg(sp + lane + 32) : 0u;
-            }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                if (vq[i] == 0ull) continue;
-                uint32_t *dst = wslots + (l0 + i) * stride;
-                if (lane < Q) dst[2 * CA + P + lane] = t[i][0];
-                if (lane + 32 < Q) dst[2 * CA + P + lane + 32] = t[i][1];
-                if (lane < P) dst[CA + lane] = t[i][2];
-                if (lane + 32 < P) dst[CA + lane + 32] = t[i][3];
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------------------------
-// fragment: steps 1-5
+// fragment: steps 1-5. V = 2 or 4 (when k + 1 is odd the host takes the tile kernel + leaf-hash kernel route instead).
 // ------------------------------------------------------------------------------------------------------------
-template <int C, int V, bool DIGEST>
+template <int C, int V>
 __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_kernel(const __grid_constant__ DctParams p) {
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
@@ -477,7 +431,7 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
     ShaMeta oth;
     const int hoff = dct_stash_offset(k);
     sha256_init(cur.H);
-    if (DIGEST) stash_init<V>(my, hoff);
+    stash_init<V>(my, hoff);
     cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
     oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
     Keystream K;
@@ -502,8 +456,8 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
                     if (g < P) {
                         vec_store<V>(mp + g, x);   // plaintext; encrypted in place below
                     } else {
-                        if (DIGEST || V == 1) vec_store<V>(mq + g, x);
-                        if (V > 1) vec_store<V>(pq + g, x);
+                        vec_store<V>(mq + g, x);
+                        vec_store<V>(pq + g, x);
                     }
                 }
                 const unsigned long long w0 = priv_word0 + (unsigned long long)s * P;
@@ -514,34 +468,25 @@ __global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_ker
                     vec_load<V>(mp + j, x);
 #pragma unroll
                     for (int t = 0; t < V; ++t) x[t] ^= ks[t];
-                    if (DIGEST || V == 1) vec_store<V>(mp + j, x);
-                    if (V > 1) vec_store<V>(pv + j, x);
+                    vec_store<V>(mp + j, x);
+                    vec_store<V>(pv + j, x);
                 }
             }
-            if (V == 1) {
-                __syncwarp();
-                warp_copy_runs<true>(wslots, p.slot_stride, P, Q, act ? reinterpret_cast<unsigned long long>(pq + P) : 0ull,
-                                     act ? reinterpret_cast<unsigned long long>(pv) : 0ull);
-                __syncwarp();
-            }
-            if (DIGEST) { cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0; }
+            cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0;
         }
-        if (DIGEST) {
 #pragma unroll 1
-            for (int it = 0; it < 2; ++it) {
-                if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-                absorb<V>(my, cur, p.one);
-                swap_streams<V>(my, hoff, cur, oth);
-            }
+        for (int it = 0; it < 2; ++it) {
+            if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
+            absorb<V>(my, cur, p.one);
+            swap_streams<V>(my, hoff, cur, oth);
         }
     }
-    if (DIGEST && L.valid) {
+    if (L.valid) {
         const size_t nl = p.leaves_per_image;
         if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
         stash_read<V>(my, hoff, cur.H);  // after an even number of swaps the private stream is the stashed one
         store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
     }
-    if (V == 1) __syncwarp();  // the next group's first copy-out reads every lane's slot
     }
 }
 

@@ -342,3 +342,34 @@ def test_digest_free_tile_kernels(orc, b, n, w, h, c, k):
     out.zero_()
     full.defragment(out, key, d_nonces, expected=full.digests)
     assert torch.equal(out, d_imgs) and int(full.flags_out.abs().sum().item()) == 0
+
+
+# Steps 1-5 run either in the fused thread-per-leaf kernel (full persistent grid, k + 1 even) or as tile kernel + leaf-hash kernel
+# (everything else); the library picks by size. Both routes must produce the same bytes and digests at any size.
+@pytest.mark.parametrize("n,w,h,c,k", [(1, 8, 8, 1, 3), (2, 264, 16, 3, 3), (1, 1032, 24, 1, 5), (3, 1920, 16, 3, 7), (2, 520, 40, 4, 1),
+                                       (1, 2056, 8, 1, 9), (1, 256, 64, 3, 31), (1, 512, 8, 4, 61), (1, 2048, 8, 3, 63)])
+def test_fused_and_split_fragment_routes_agree(orc, b, n, w, h, c, k, monkeypatch):
+    key, nonce = synth.key_nonce(w + k)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=11 * w + i + k) for i in range(n)])
+    d_imgs = torch.from_numpy(imgs).cuda()
+    d_nonces = torch.from_numpy(nonces).cuda()
+    fused, split = b.DctBatch(n, w, h, c, k), b.DctBatch(n, w, h, c, k)
+    for t in (fused.priv, fused.pub, fused.digests, split.priv, split.pub, split.digests):
+        t.fill_(0x5A)
+    monkeypatch.setenv("FEDS_FRAGMENT_PATH", "fused")
+    fused.fragment(d_imgs, key, d_nonces)
+    monkeypatch.setenv("FEDS_FRAGMENT_PATH", "split")
+    split.fragment(d_imgs, key, d_nonces)
+    monkeypatch.delenv("FEDS_FRAGMENT_PATH")
+    torch.cuda.synchronize()
+    assert torch.equal(fused.priv, split.priv) and torch.equal(fused.pub, split.pub) and torch.equal(fused.digests, split.digests)
+    # and they are the oracle's for these coefficient bytes (image 0)
+    pv, pb = fused.priv[:fused.priv_bytes].cpu().numpy(), fused.pub[:fused.pub_bytes].cpu().numpy()
+    coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[0].tobytes())
+    assert np.abs(coef - orc.dct_coefficients(imgs[0])).max() <= TOL
+    p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[0].tobytes())
+    assert (p2 == pv).all() and (q2 == pb).all() and d2 == fused.digests[:64].cpu().numpy().tobytes()
+    out = torch.zeros_like(d_imgs)
+    fused.defragment(out, key, d_nonces, expected=split.digests)
+    assert torch.equal(out, d_imgs) and int(fused.flags_out.abs().sum().item()) == 0
