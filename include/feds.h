@@ -119,6 +119,12 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
                                 uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
                                 size_t workspace_bytes, feds_stream_t stream);
 
+/* feds_verify_dwt — as feds_verify_dct for the DWT path's fragments (2048-byte leaves of each fragment stream); no key needed.
+ * Workspace as for feds_defragment_dwt. */
+feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,
+                            const uint8_t *d_expected_digests, uint32_t *d_verify_flags, void *d_workspace,
+                            size_t workspace_bytes, feds_stream_t stream);
+
 /*
  * Batched DCT entry points ("series of images"): n_images images of identical shape, image i at
  * d_images + i*image_stride, fragments at d_private + i*private_stride / d_public + i*public_stride, digests at

@@ -26,7 +26,7 @@ SYMBOLS = [
     "feds_fragment_dct_batch", "feds_defragment_dct_batch",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
-    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch",
+    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
 ]
 
@@ -64,6 +64,7 @@ def _load():
     lib.feds_defragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_defragment_dct_host.argtypes = [vp, vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
     lib.feds_verify_dct.argtypes = [vp, vp, i, i, i, i, vp, vp, vp, sz, vp]
+    lib.feds_verify_dwt.argtypes = lib.feds_verify_dct.argtypes
     lib.feds_verify_dct_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, vp, vp, vp, sz, vp]
     lib.feds_aes128_ctr.argtypes = [vp, vp, sz, u8p, u8p, vp]
     lib.feds_sha256_merkle_workspace_bytes.restype = sz
@@ -77,7 +78,7 @@ def _load():
     lib.feds_debug_zigzag_host.argtypes = [vp]
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
                  "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host",
-                 "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch"]:
+                 "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt"]:
         getattr(lib, name).restype = i
     return lib
 
@@ -168,6 +169,16 @@ def verify_dct(priv, pub, w, h, c, k, expected, stream=None, workspace=None):
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
     _check(lib.feds_verify_dct(_ptr(priv), _ptr(pub), w, h, c, k, _ptr(expected), _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)),
            "feds_verify_dct")
+    return flags
+
+
+def verify_dwt(priv, pub, w, h, c, levels, expected, stream=None, workspace=None):
+    """feds_verify_dwt: integrity of the DWT fragments against their digest pair, no key needed -> flags tensor [1]."""
+    dev = priv.device
+    flags = torch.zeros(1, dtype=torch.int32, device=dev)
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
+    _check(lib.feds_verify_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, _ptr(expected), _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)),
+           "feds_verify_dwt")
     return flags
 
 

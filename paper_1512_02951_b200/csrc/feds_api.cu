@@ -705,6 +705,25 @@ feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_publi
     return FEDS_OK;
 }
 
+feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,
+                            const uint8_t *d_expected_digests, uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                            feds_stream_t stream) {
+    if (w <= 0 || h <= 0) return FEDS_ERR_BAD_DIMS;
+    if (!chan_ok(c) || levels < 1 || levels > 6) return FEDS_ERR_BAD_PARAM;
+    if (!dwt_dims_ok(w, h, levels)) return FEDS_ERR_BAD_DIMS;
+    if (!d_private || !d_public || !d_expected_digests || !d_verify_flags || !d_workspace) return FEDS_ERR_NULL_POINTER;
+    if (misaligned(d_private) || misaligned(d_public) || misaligned(d_expected_digests) || misaligned(d_workspace)) return FEDS_ERR_MISALIGNED;
+    const DwtPlan pl = dwt_plan(w, h, c, levels);
+    if (workspace_bytes < pl.per_image) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    uint8_t *roots = ws + pl.per_image - 64;
+    const feds_status st = dwt_digests(d_private, d_public, pl, ws + pl.planes_bytes, roots, stream);
+    if (st != FEDS_OK) return st;
+    compare_digests_kernel<<<1, 32, 0, stream>>>(roots, d_expected_digests, d_verify_flags, 1);
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ stream primitives
 feds_status feds_aes128_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16], const uint8_t nonce[16],
                             feds_stream_t stream) {

@@ -56,6 +56,11 @@ def test_dwt_verify_flags(orc, b):
     q2 = pub.clone(); q2[-2] ^= 0x10
     _, flags = b.defragment_dwt(priv, q2, 256, 128, 3, 3, key, nonce, expected=dg)
     assert int(flags.item()) == 2
+    # the same check without the key (feds_verify_dwt)
+    assert int(b.verify_dwt(priv, pub, 256, 128, 3, 3, dg).item()) == 0
+    assert int(b.verify_dwt(p2, pub, 256, 128, 3, 3, dg).item()) == 1
+    assert int(b.verify_dwt(priv, q2, 256, 128, 3, 3, dg).item()) == 2
+    assert int(b.verify_dwt(p2, q2, 256, 128, 3, 3, dg).item()) == 3
 
 
 def test_config4_full_size(orc, b):
