@@ -23,10 +23,7 @@ namespace feds {
 
 __device__ const AesTables g_aes = make_aes_tables();
 
-#ifndef FEDS_FRAG_THREADS
-#define FEDS_FRAG_THREADS 512
-#endif
-constexpr int DCT_THREADS = FEDS_FRAG_THREADS;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
+constexpr int DCT_THREADS = 512;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
 constexpr int DCT_CTAS_PER_SM = 1;
 constexpr size_t DCT_SMEM_MAX = 227 * 1024;
 constexpr int AES_TABLE_WORDS = 1024;
@@ -340,14 +337,7 @@ __device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s, const uint32_
 #pragma unroll
             for (int t = 0; t < VA; ++t) w[i + t] = bswap32(x[t]);
         }
-#if !defined(FEDS_SHA_FMA_ADDS) || FEDS_SHA_FMA_ADDS  // default: +6 % on B200 (ALU pipe is the binding unit, FMA pipe idles)
         sha256_compress_rolled_fma(s.H, w, one);
-#elif !defined(FEDS_SHA_ROLLED) || FEDS_SHA_ROLLED
-        (void)one;
-        sha256_compress_rolled(s.H, w);
-#else
-        sha256_compress(s.H, w);
-#endif
         ptr += 16;
         cnt -= 16;
     }

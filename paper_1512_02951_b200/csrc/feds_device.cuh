@@ -223,11 +223,7 @@ inline void aes128_expand_key_host(const uint8_t key[16], uint32_t rk[44], const
 template <typename TabPtr, typename RkPtr>
 FEDS_HD void aes128_encrypt(const TabPtr T, const RkPtr rk, uint32_t (&s)[4]) {
     uint32_t s0 = s[0] ^ rk[0], s1 = s[1] ^ rk[1], s2 = s[2] ^ rk[2], s3 = s[3] ^ rk[3];
-#if defined(FEDS_AES_ROLLED) && FEDS_AES_ROLLED
-#pragma unroll 1
-#else
 #pragma unroll
-#endif
     for (int r = 1; r < 10; ++r) {
         const uint32_t t0 = T[0 * 256 + (s0 & 0xff)] ^ T[1 * 256 + ((s1 >> 8) & 0xff)] ^ T[2 * 256 + ((s2 >> 16) & 0xff)] ^
                             T[3 * 256 + (s3 >> 24)] ^ rk[4 * r + 0];
