@@ -308,7 +308,7 @@ def main():
     prof_frag, prof_defrag = [], []
 
     if kind == "dct":
-        nonces = sharding.nonces_for(nonce, rank * n, n)   # weak scaling: rank r owns global images [r*n, (r+1)*n)
+        nonces = sharding.nonces_for(nonce, rank * n, n, priv_bytes=B.dct_private_bytes(w, h, c, kl))   # weak scaling: rank r owns global images [r*n, (r+1)*n)
         d_nonces = torch.from_numpy(nonces).to(dev)
         d_imgs = synth.image_batch_torch(n, w, h, c, seed=3000 + 1000 * rank, device=dev, rectangles=rects)
         d_out = torch.empty_like(d_imgs)

@@ -45,6 +45,11 @@ typedef enum {
 #define FEDS_FLAG_NONE 0u
 #define FEDS_FLAG_NO_DIGEST 1u /* skip step 5 (SHA-256 Merkle digests): the report's own selective encryption (DCT + select + AES,
                                   P:488-494), HBM-bound. d_digests is not written; defragment does not verify. */
+/* Route overrides (tests and profiling; results are byte-identical on every route). Without them the library picks the
+ * route from the shape alone. A forced route that does not support the shape returns FEDS_ERR_BAD_PARAM. */
+#define FEDS_FLAG_FORCE_FUSED 2u /* DCT with digests: the warp-specialised fused kernel (needs (w/8) % 8 == 0 and k + 1 even) */
+#define FEDS_FLAG_FORCE_SPLIT 4u /* DCT with digests: digest-free tile kernel + leaf-hash kernel */
+#define FEDS_FLAG_DWT_TILED 8u   /* DWT: the tiled shared-memory level kernels instead of the register-streaming ones */
 
 const char *feds_status_string(feds_status s);
 int feds_last_cuda_error(void); /* cudaError_t of the most recent FEDS_ERR_CUDA on this thread, else 0 */
@@ -126,10 +131,30 @@ feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, i
                             size_t workspace_bytes, feds_stream_t stream);
 
 /*
+ * Batched DWT entry points: n_images images of identical shape at the given byte strides (multiples of 16), one nonce per image
+ * in the DEVICE array d_nonces (uint8[n_images][16], non-overlapping counter ranges as for the DCT batch), digests at
+ * d_digests + 64 i, verify flags at d_verify_flags + i. Every level kernel, the AES-CTR pass and the leaf hashing span the
+ * whole batch in one launch each. Workspace: n_images * feds_workspace_bytes(w, h, c, levels, 1).
+ * flags: FEDS_FLAG_NONE or FEDS_FLAG_DWT_TILED.
+ */
+feds_status feds_fragment_dwt_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int levels,
+                                    const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private, size_t private_stride,
+                                    uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                                    size_t workspace_bytes, unsigned flags, feds_stream_t stream);
+feds_status feds_defragment_dwt_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                      int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *d_nonces,
+                                      const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                      uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                      feds_stream_t stream);
+
+/*
  * Batched DCT entry points ("series of images"): n_images images of identical shape, image i at
  * d_images + i*image_stride, fragments at d_private + i*private_stride / d_public + i*public_stride, digests at
  * d_digests + 64 i, verify flags at d_verify_flags + i. Every image is an independent CTR message with its own
  * nonce ("different IV for each input matrix"): d_nonces is a DEVICE array uint8[n_images][16].
+ * The counter ranges must not overlap: every image uses the counter blocks [nonce_i, nonce_i + ceil(private_bytes / 16)) mod 2^128
+ * under the one key, so any two nonces of a batch (and of every other batch under that key) must differ by at least that many
+ * blocks -- overlapping ranges reuse keystream (a two-time pad). The library cannot check this across calls; it is the caller's duty.
  * One launch per stage spans the whole batch. Strides are in bytes, multiples of 16, >= the per-image size.
  * Workspace: n_images * feds_workspace_bytes(...).
  */
@@ -203,19 +228,6 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
  * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.
  */
 void feds_profile_events(void *ev_start, void *ev_stop);
-
-/*
- * Host-side arithmetic self-checks of the device building blocks (the same __host__ __device__ functions the
- * kernels call), usable without a GPU. Not part of the data path.
- *   feds_debug_sha256_host   : SHA-256 of a host buffer through the kernels' compression function.
- *   feds_debug_aes128_host   : one AES-128 block through the kernels' T-table rounds.
- *   feds_debug_dct8x8_host   : forward (inverse=0) / inverse (inverse=1) 8x8 float32 transform, row-major.
- *   feds_debug_zigzag_host   : the kernels' zigzag table, out[z] = 8*row + col.
- */
-void feds_debug_sha256_host(const uint8_t *msg, size_t n, uint8_t out[32]);
-void feds_debug_aes128_host(const uint8_t key[16], const uint8_t in[16], uint8_t out[16]);
-void feds_debug_dct8x8_host(const float in[64], float out[64], int inverse);
-void feds_debug_zigzag_host(int out[64]);
 
 #ifdef __cplusplus
 }

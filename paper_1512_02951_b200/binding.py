@@ -13,17 +13,20 @@ LIB_PATH = os.environ.get("FEDS_LIB_PATH") or os.path.join(_HERE, "libfeds.so")
 
 FLAG_NONE = 0
 FLAG_NO_DIGEST = 1
+FLAG_FORCE_FUSED = 2
+FLAG_FORCE_SPLIT = 4
+FLAG_DWT_TILED = 8
 
 STATUS = {0: "FEDS_OK", 1: "FEDS_ERR_NULL_POINTER", 2: "FEDS_ERR_BAD_DIMS", 3: "FEDS_ERR_BAD_PARAM",
           4: "FEDS_ERR_WORKSPACE_TOO_SMALL", 5: "FEDS_ERR_CUDA", 6: "FEDS_ERR_MISALIGNED"}
 
-# every symbol include/feds.h declares
+# every symbol include/feds.h and include/feds_debug.h declare
 SYMBOLS = [
     "feds_status_string", "feds_last_cuda_error", "feds_merkle_params",
     "feds_dct_private_bytes", "feds_dct_public_bytes", "feds_dwt_private_bytes", "feds_dwt_public_bytes",
     "feds_workspace_bytes",
     "feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
-    "feds_fragment_dct_batch", "feds_defragment_dct_batch",
+    "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
     "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
@@ -57,6 +60,8 @@ def _load():
     lib.feds_defragment_dwt.argtypes = lib.feds_defragment_dct.argtypes
     lib.feds_fragment_dct_batch.argtypes = [vp, i, sz, i, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, C.c_uint, vp]
     lib.feds_defragment_dct_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, u8p, vp, vp, vp, sz, vp, vp, sz, C.c_uint, vp]
+    lib.feds_fragment_dwt_batch.argtypes = lib.feds_fragment_dct_batch.argtypes
+    lib.feds_defragment_dwt_batch.argtypes = lib.feds_defragment_dct_batch.argtypes
     lib.feds_fragment_dct_host_scratch_bytes.restype = sz
     lib.feds_fragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_fragment_dct_host.argtypes = [vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
@@ -77,7 +82,8 @@ def _load():
     lib.feds_debug_dct8x8_host.argtypes = [vp, vp, i]
     lib.feds_debug_zigzag_host.argtypes = [vp]
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
-                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dct_host", "feds_defragment_dct_host",
+                 "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
+                 "feds_fragment_dct_host", "feds_defragment_dct_host",
                  "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt"]:
         getattr(lib, name).restype = i
     return lib
@@ -98,6 +104,23 @@ def _ptr(t):
 def _stream(stream):
     s = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(s.cuda_stream)
+
+
+def _k16(b):
+    """key / nonce: exactly 16 bytes (the library reads 16 bytes from the pointer it is given)."""
+    b = bytes(b)
+    if len(b) != 16:
+        raise ValueError("key and nonce must be 16 bytes, got %d" % len(b))
+    return b
+
+
+def _on_stream(stream, *tensors):
+    """Tensors allocated here on torch's current stream but used by kernels enqueued on `stream`: tell the caching allocator,
+    so that the memory is not handed to other work while those kernels may still run."""
+    if stream is not None and stream != torch.cuda.current_stream():
+        for t in tensors:
+            if t is not None and t.is_cuda:
+                t.record_stream(stream)
 
 
 def merkle_params():
@@ -146,7 +169,8 @@ def fragment_dct(image, k, key, nonce, stream=None, workspace=None):
     pub = _u8(dct_public_bytes(w, h, c, k), dev)
     dg = _u8(64, dev)
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
-    _check(lib.feds_fragment_dct(_ptr(image), w, h, c, k, bytes(key), bytes(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
+    _on_stream(stream, priv, pub, dg, ws)
+    _check(lib.feds_fragment_dct(_ptr(image), w, h, c, k, _k16(key), _k16(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
                                  ws.numel(), _stream(stream)), "feds_fragment_dct")
     return priv[:dct_private_bytes(w, h, c, k)], pub[:dct_public_bytes(w, h, c, k)], dg
 
@@ -157,7 +181,8 @@ def defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=None, stream=None
     out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
     flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
-    _check(lib.feds_defragment_dct(_ptr(priv), _ptr(pub), w, h, c, k, bytes(key), bytes(nonce), _ptr(expected), _ptr(out),
+    _on_stream(stream, out, flags, ws)
+    _check(lib.feds_defragment_dct(_ptr(priv), _ptr(pub), w, h, c, k, _k16(key), _k16(nonce), _ptr(expected), _ptr(out),
                                    _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dct")
     return out, flags
 
@@ -167,6 +192,7 @@ def verify_dct(priv, pub, w, h, c, k, expected, stream=None, workspace=None):
     dev = priv.device
     flags = torch.zeros(1, dtype=torch.int32, device=dev)
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _on_stream(stream, flags, ws)
     _check(lib.feds_verify_dct(_ptr(priv), _ptr(pub), w, h, c, k, _ptr(expected), _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)),
            "feds_verify_dct")
     return flags
@@ -177,6 +203,7 @@ def verify_dwt(priv, pub, w, h, c, levels, expected, stream=None, workspace=None
     dev = priv.device
     flags = torch.zeros(1, dtype=torch.int32, device=dev)
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
+    _on_stream(stream, flags, ws)
     _check(lib.feds_verify_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, _ptr(expected), _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)),
            "feds_verify_dwt")
     return flags
@@ -189,7 +216,8 @@ def fragment_dwt(image, levels, key, nonce, stream=None, workspace=None):
     pub = _u8(dwt_public_bytes(w, h, c, levels), dev)
     dg = _u8(64, dev)
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
-    _check(lib.feds_fragment_dwt(_ptr(image), w, h, c, levels, bytes(key), bytes(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
+    _on_stream(stream, priv, pub, dg, ws)
+    _check(lib.feds_fragment_dwt(_ptr(image), w, h, c, levels, _k16(key), _k16(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
                                  ws.numel(), _stream(stream)), "feds_fragment_dwt")
     return priv[:dwt_private_bytes(w, h, c, levels)], pub[:dwt_public_bytes(w, h, c, levels)], dg
 
@@ -199,7 +227,8 @@ def defragment_dwt(priv, pub, w, h, c, levels, key, nonce, expected=None, stream
     out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
     flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
     ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, levels, True), dev)
-    _check(lib.feds_defragment_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, bytes(key), bytes(nonce), _ptr(expected), _ptr(out),
+    _on_stream(stream, out, flags, ws)
+    _check(lib.feds_defragment_dwt(_ptr(priv), _ptr(pub), w, h, c, levels, _k16(key), _k16(nonce), _ptr(expected), _ptr(out),
                                    _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dwt")
     return out, flags
 
@@ -209,7 +238,8 @@ def aes128_ctr(data, key, nonce, out=None, stream=None):
     data = data.contiguous().view(-1)
     if out is None:
         out = torch.empty_like(data)
-    _check(lib.feds_aes128_ctr(_ptr(data), _ptr(out), data.numel(), bytes(key), bytes(nonce), _stream(stream)), "feds_aes128_ctr")
+    _on_stream(stream, out)
+    _check(lib.feds_aes128_ctr(_ptr(data), _ptr(out), data.numel(), _k16(key), _k16(nonce), _stream(stream)), "feds_aes128_ctr")
     return out
 
 
@@ -219,6 +249,7 @@ def sha256_merkle(data, stream=None, workspace=None):
     root = _u8(32, data.device)
     need = lib.feds_sha256_merkle_workspace_bytes(data.numel())
     ws = workspace if workspace is not None else _u8(max(need, 16), data.device)
+    _on_stream(stream, root, ws)
     _check(lib.feds_sha256_merkle(_ptr(data) if data.numel() else None, data.numel(), _ptr(root), _ptr(ws), ws.numel(), _stream(stream)),
            "feds_sha256_merkle")
     return root
@@ -240,14 +271,14 @@ class DctBatch:
 
     def fragment(self, images, key, d_nonces, flags=FLAG_NONE, stream=None):
         assert images.is_cuda and images.dtype == torch.uint8 and images.is_contiguous() and images.numel() == self.n * self.image_bytes
-        _check(lib.feds_fragment_dct_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, self.k, bytes(key),
+        _check(lib.feds_fragment_dct_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, self.k, _k16(key),
                                            _ptr(d_nonces), _ptr(self.priv), self.priv_bytes, _ptr(self.pub), self.pub_bytes,
                                            _ptr(self.digests), _ptr(self.ws), self.ws.numel(), flags, _stream(stream)),
                "feds_fragment_dct_batch")
 
     def defragment(self, images_out, key, d_nonces, expected=None, flags=FLAG_NONE, stream=None):
         _check(lib.feds_defragment_dct_batch(_ptr(self.priv), self.priv_bytes, _ptr(self.pub), self.pub_bytes, self.n, self.w, self.h,
-                                             self.c, self.k, bytes(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
+                                             self.c, self.k, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
                                              self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
                                              _stream(stream)), "feds_defragment_dct_batch")
 
@@ -261,12 +292,42 @@ class DctBatch:
         return self.flags_out
 
 
+class DwtBatch:
+    """Pre-allocated buffers for feds_fragment_dwt_batch / feds_defragment_dwt_batch on n images of one shape."""
+
+    def __init__(self, n, w, h, c, levels, device="cuda"):
+        self.n, self.w, self.h, self.c, self.levels = n, w, h, c, levels
+        self.image_bytes = w * h * c
+        self.priv_bytes = dwt_private_bytes(w, h, c, levels)
+        self.pub_bytes = dwt_public_bytes(w, h, c, levels)
+        self.priv_stride = (self.priv_bytes + 15) // 16 * 16
+        self.pub_stride = (self.pub_bytes + 15) // 16 * 16
+        self.priv = _u8(n * self.priv_stride, device)
+        self.pub = _u8(n * self.pub_stride, device)
+        self.digests = _u8(n * 64, device)
+        self.ws = _u8(n * workspace_bytes(w, h, c, levels, True), device)
+        self.flags_out = torch.zeros(n, dtype=torch.int32, device=device)
+
+    def fragment(self, images, key, d_nonces, flags=FLAG_NONE, stream=None):
+        assert images.is_cuda and images.dtype == torch.uint8 and images.is_contiguous() and images.numel() == self.n * self.image_bytes
+        _check(lib.feds_fragment_dwt_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, self.levels, _k16(key),
+                                           _ptr(d_nonces), _ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride,
+                                           _ptr(self.digests), _ptr(self.ws), self.ws.numel(), flags, _stream(stream)),
+               "feds_fragment_dwt_batch")
+
+    def defragment(self, images_out, key, d_nonces, expected=None, flags=FLAG_NONE, stream=None):
+        _check(lib.feds_defragment_dwt_batch(_ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, self.n, self.w, self.h,
+                                             self.c, self.levels, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
+                                             self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
+                                             _stream(stream)), "feds_defragment_dwt_batch")
+
+
 def fragment_dct_host(h_images, w, h, c, k, key, h_nonces, h_priv, h_pub, h_digests, images_per_chunk, d_scratch, streams,
                       flags=FLAG_NONE):
     """feds_fragment_dct_host: pinned host tensors in/out, staged over `streams` (torch.cuda.Stream list)."""
     n = h_images.numel() // (w * h * c)
     arr = (C.c_void_p * len(streams))(*[s.cuda_stream for s in streams])
-    _check(lib.feds_fragment_dct_host(_ptr(h_images), n, w, h, c, k, bytes(key), _ptr(h_nonces), _ptr(h_priv), _ptr(h_pub),
+    _check(lib.feds_fragment_dct_host(_ptr(h_images), n, w, h, c, k, _k16(key), _ptr(h_nonces), _ptr(h_priv), _ptr(h_pub),
                                       _ptr(h_digests), images_per_chunk, _ptr(d_scratch), d_scratch.numel(), arr, len(streams), flags),
            "feds_fragment_dct_host")
 
@@ -279,7 +340,7 @@ def defragment_dct_host(h_priv, h_pub, n, w, h, c, k, key, h_nonces, h_expected,
                         streams, flags=FLAG_NONE):
     """feds_defragment_dct_host: pinned host tensors in/out, staged over `streams`."""
     arr = (C.c_void_p * len(streams))(*[s.cuda_stream for s in streams])
-    _check(lib.feds_defragment_dct_host(_ptr(h_priv), _ptr(h_pub), n, w, h, c, k, bytes(key), _ptr(h_nonces), _ptr(h_expected),
+    _check(lib.feds_defragment_dct_host(_ptr(h_priv), _ptr(h_pub), n, w, h, c, k, _k16(key), _ptr(h_nonces), _ptr(h_expected),
                                         _ptr(h_images_out), _ptr(h_flags), images_per_chunk, _ptr(d_scratch), d_scratch.numel(), arr,
                                         len(streams), flags), "feds_defragment_dct_host")
 

@@ -8,42 +8,41 @@
 #include <cstring>
 
 #include "../../include/feds.h"
+#include "../../include/feds_debug.h"
 #include "feds_dct.cuh"
-#include "feds_dct_tile.cuh"
 #include "feds_device.cuh"
 #include "feds_dwt.cuh"
-#include "feds_dwt_fast.cuh"
-#include "feds_hash.cuh"
+#include "feds_host.h"
 
 using namespace feds;
 
 namespace {
-
 thread_local int t_last_cuda_error = 0;
 thread_local cudaEvent_t t_prof_start = nullptr, t_prof_stop = nullptr;
-constexpr AesTables h_aes = make_aes_tables();
-constexpr ZigzagTable h_zigzag = make_zigzag();
+}  // namespace
 
-inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
-
+namespace feds {
 feds_status cuda_fail(cudaError_t e) {
     t_last_cuda_error = (int)e;
     return FEDS_ERR_CUDA;
 }
-#define FEDS_CUDA(call)                                   \
-    do {                                                  \
-        cudaError_t e__ = (call);                         \
-        if (e__ != cudaSuccess) return cuda_fail(e__);    \
-    } while (0)
-#define FEDS_LAUNCH_CHECK() FEDS_CUDA(cudaGetLastError())
-
-// SMs of the current device (the persistent DCT kernels launch one CTA per SM); asked per call, nothing is cached
+// SMs of the current device; asked per call, nothing is cached
 int sm_count() {
     int dev = 0, n = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
     return n;
 }
+cudaEvent_t prof_start_event() { return t_prof_start; }
+cudaEvent_t prof_stop_event() { return t_prof_stop; }
+}  // namespace feds
+
+namespace {
+
+constexpr AesTables h_aes = make_aes_tables();
+constexpr ZigzagTable h_zigzag = make_zigzag();
+
+inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
 bool dct_dims_ok(int w, int h) { return w > 0 && h > 0 && (w % 8) == 0 && (h % 8) == 0; }
 bool chan_ok(int c) { return c == 1 || c == 3 || c == 4; }
@@ -70,74 +69,6 @@ unsigned dct_leaves(int w, int h, int c) { return (unsigned)c * (unsigned)(h / 8
 void nonce_to_be(const uint8_t nonce[16], uint32_t out[4]) {
     for (int i = 0; i < 4; ++i)
         out[i] = ((uint32_t)nonce[4 * i] << 24) | ((uint32_t)nonce[4 * i + 1] << 16) | ((uint32_t)nonce[4 * i + 2] << 8) | nonce[4 * i + 3];
-}
-
-// Reduce level-0 digests [tree][n0][32] (tree stride = n0*32) to roots written at roots + tree*root_stride.
-// `scratch` holds the intermediate levels. n_trees trees of identical shape.
-// wide levels of n_trees equal trees: one thread per node until at most TAIL_MAX_IN digests per tree remain
-feds_status reduce_wide(const uint8_t *&in, unsigned &n, unsigned n_trees, uint8_t *&sc, int skip_odd, cudaStream_t stream) {
-    MerkleLevelParams mp{};
-    mp.n_trees = n_trees;
-    mp.odd_trees_only_if_nonempty = skip_odd;
-    mp.one = 1u;
-    while (n > TAIL_MAX_IN) {
-        const unsigned m = (n + FANOUT - 1) / FANOUT;
-        mp.in = in; mp.n_in = n; mp.n_out = m; mp.in_tree_stride = (size_t)n * 32;
-        mp.out = sc; mp.out_tree_stride = (size_t)m * 32;
-        const unsigned long long threads = (unsigned long long)n_trees * m;
-        merkle_level_kernel<<<(unsigned)((threads + HASH_THREADS - 1) / HASH_THREADS), HASH_THREADS, 0, stream>>>(mp);
-        FEDS_LAUNCH_CHECK();
-        in = sc;
-        sc += (size_t)n_trees * m * 32;
-        n = m;
-    }
-    return FEDS_OK;
-}
-
-feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
-                     int skip_odd, cudaStream_t stream) {
-    const uint8_t *in = level0;
-    uint8_t *sc = scratch;
-    unsigned n = n0;
-    feds_status st = reduce_wide(in, n, n_trees, sc, skip_odd, stream);
-    if (st != FEDS_OK) return st;
-    if (n > 1) {  // the top (<= 4096 digests per tree): one CTA per tree, up to three levels in one launch
-        MerkleLevelParams mp{};
-        mp.n_trees = n_trees; mp.odd_trees_only_if_nonempty = skip_odd; mp.one = 1u;
-        mp.in = in; mp.n_in = n; mp.n_out = 1; mp.in_tree_stride = (size_t)n * 32;
-        mp.out = roots; mp.out_tree_stride = root_stride;
-        merkle_tail_kernel<<<n_trees, TAIL_THREADS, 0, stream>>>(mp);
-        FEDS_LAUNCH_CHECK();
-    }
-    return FEDS_OK;
-}
-
-// two single trees of different shapes (DWT private / public): wide levels separately, both tops in one launch
-feds_status run_two_trees(const uint8_t *l0a, unsigned na, uint8_t *sca, uint8_t *roota, const uint8_t *l0b, unsigned nb, uint8_t *scb,
-                          uint8_t *rootb, cudaStream_t stream) {
-    const uint8_t *ina = l0a, *inb = l0b;
-    feds_status st = reduce_wide(ina, na, 1, sca, 0, stream);
-    if (st != FEDS_OK) return st;
-    st = reduce_wide(inb, nb, 1, scb, 0, stream);
-    if (st != FEDS_OK) return st;
-    if (na <= 1 && nb <= 1) return FEDS_OK;  // one-leaf trees: the leaf kernel already wrote the roots
-    MerkleLevelParams mp{};
-    mp.one = 1u; mp.n_out = 1;
-    unsigned ctas = 0;
-    if (na > 1) { mp.n_trees = 1; mp.in = ina; mp.n_in = na; mp.in_tree_stride = 0; mp.out = roota; mp.out_tree_stride = 0; ctas = 1; }
-    if (nb > 1) {
-        if (ctas == 0) { mp.n_trees = 1; mp.in = inb; mp.n_in = nb; mp.out = rootb; ctas = 1; }
-        else { mp.in2 = inb; mp.n_in2 = nb; mp.out2 = rootb; ctas = 2; }
-    }
-    merkle_tail_kernel<<<ctas, TAIL_THREADS, 0, stream>>>(mp);
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
-}
-
-template <typename K>
-feds_status set_smem(K kernel, size_t bytes) {
-    FEDS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    return FEDS_OK;
 }
 
 struct DctPlan {
@@ -171,91 +102,29 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.slot_stride = dct_slot_words(k);
     p.one = 1u;
     p.n_groups = (unsigned)((p.total_leaves + 31) / 32);
+    p.ws_n_sg = (unsigned)(((unsigned long long)n_images * p.nbr * p.nlr + 31) / 32);
+    {   // the hash warps fetch 16 words at a time: the worker must be allowed far enough ahead to cover one fetch (feds_dct_ws.cuh)
+        const int wq = (63 - k) > 0 ? (63 - k) : (k + 1);
+        p.ws_ahead = std::max(2, (16 + wq - 1) / wq + 1);
+    }
+    p.c128 = 128u;
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
     aes128_expand_key_host(key, p.rk, h_aes);
 }
 
-template <template <int, int> class Launcher>
-feds_status dispatch_cv(const DctParams &p, int c, cudaStream_t stream) {
-    const int V = dct_vec_width(p.k);
-#define FEDS_V(CC)                                                                  \
-    (V == 4 ? Launcher<CC, 4>::go(p, stream) : V == 2 ? Launcher<CC, 2>::go(p, stream) : Launcher<CC, 1>::go(p, stream))
-    return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
-#undef FEDS_V
-}
-
-template <typename Kernel>
-feds_status launch_dct(Kernel kernel, const DctParams &p, cudaStream_t stream, int max_threads = DCT_THREADS) {
-    // persistent: one CTA per SM, its warps stride over the leaf groups. 16 warps unless their slots exceed the SM's
-    // shared memory (k >= 32: the padding slack grows), then 8.
-    int threads = max_threads;
-    size_t smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4;
-    if (smem > DCT_SMEM_MAX) { threads = 256; smem = (size_t)(AES_TABLE_WORDS + threads * p.slot_stride) * 4; }
-    const unsigned grid = std::min<unsigned>(p.n_groups, (unsigned)sm_count());
-    feds_status s = set_smem(kernel, smem);
-    if (s != FEDS_OK) return s;
-    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    kernel<<<grid, threads, smem, stream>>>(p);
-    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
-}
-
-// digest-free path: one persistent CTA per SM, GROUPS tile groups inside it (feds_dct_tile.cuh)
-template <int C, typename Kernel>
-feds_status launch_dct_tile(Kernel kernel, const DctParams &p, cudaStream_t stream, bool record_start = true) {
-    constexpr int TB = TileShape<C>::TB, GROUPS = TileShape<C>::GROUPS;
-    const size_t smem = tile_smem_bytes<C>(p.k);
-    feds_status s = set_smem(kernel, smem);
-    if (s != FEDS_OK) return s;
-    const unsigned long long tiles = (unsigned long long)p.n_images * p.nbr * ((p.nbc + TB - 1) / TB);
-    const unsigned grid = (unsigned)std::min<unsigned long long>((tiles + GROUPS - 1) / GROUPS, (unsigned long long)sm_count());
-    if (t_prof_start && record_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    kernel<<<grid, TileShape<C>::CTA, smem, stream>>>(p);
-    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
-}
-
-// leaf digests of fragments as they lie in memory (feds_dct_tile.cuh): the verification half of a verified defragment
-feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream) {
-    const unsigned long long threads = 2 * p.total_leaves;
-    const unsigned grid = (unsigned)((threads + LEAFHASH_THREADS - 1) / LEAFHASH_THREADS);
-    if (c == 1) dct_leaves_hash_kernel<1><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);
-    else if (c == 3) dct_leaves_hash_kernel<3><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);
-    else dct_leaves_hash_kernel<4><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
-}
-
-template <int C, int V> struct FragDigest { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct(fragment_dct_kernel<C, V>, p, s); } };
-template <int C, int V> struct FragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(fragment_dct_tile_kernel<C, V>, p, s); } };
-template <int C, int V> struct DefragPlain { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(defragment_dct_tile_kernel<C, V>, p, s); } };
-template <int C, int V> struct DefragAfterHash { static feds_status go(const DctParams &p, cudaStream_t s) { return launch_dct_tile<C>(defragment_dct_tile_kernel<C, V>, p, s, false); } };
-
-feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream) { return dispatch_cv<FragPlain>(p, c, stream); }
-// the fused kernel exists for V = 4 and V = 2 only
-feds_status launch_fragment_fused(const DctParams &p, int c, cudaStream_t stream) {
-    const int V = dct_vec_width(p.k);
-#define FEDS_V(CC) (V == 4 ? FragDigest<CC, 4>::go(p, stream) : FragDigest<CC, 2>::go(p, stream))
-    return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
-#undef FEDS_V
-}
-// Steps 1-5 in one fused kernel pay when its persistent grid is full (16 warps per SM for at least two rounds) and the runs
-// are 8- or 16-byte multiples; otherwise the digest-free tile kernel followed by the leaf-hash kernel of what it wrote is
-// faster (measured: 11 % at 512^2, 3 % at one 4096^2 image, 2-4 % for odd k + 1 at any size; 3 % slower at cfg3).
-bool fragment_fused_pays(const DctParams &p) {
-    if (dct_vec_width(p.k) == 1) return false;
-    if (const char *force = getenv("FEDS_FRAGMENT_PATH")) {   // test hook: "fused" | "split"
-        if (force[0] == 'f') return true;
-        if (force[0] == 's') return false;
-    }
-    return p.n_groups >= 2u * (DCT_THREADS / 32) * (unsigned)sm_count();
-}
-feds_status launch_defragment(const DctParams &p, int c, cudaStream_t stream, bool after_hash = false) {
-    return after_hash ? dispatch_cv<DefragAfterHash>(p, c, stream) : dispatch_cv<DefragPlain>(p, c, stream);
+// Which route fragments with digests. The warp-specialised fused kernel (feds_dct_ws.cuh) needs whole 8-block leaves and
+// 8/16-byte runs, and pays once its persistent grid is full; everything else runs as the digest-free tile kernel followed
+// by the leaf-hash kernel over what it wrote.
+constexpr unsigned DCT_FLAGS = FEDS_FLAG_NO_DIGEST | FEDS_FLAG_FORCE_FUSED | FEDS_FLAG_FORCE_SPLIT;
+enum class Route { Fused, Split, Unsupported };
+Route pick_route(const DctParams &p, int c, unsigned flags) {
+    const bool ws_ok = dct_ws_supported(p, c);
+    if (flags & FEDS_FLAG_FORCE_FUSED) return ws_ok ? Route::Fused : Route::Unsupported;
+    if (flags & FEDS_FLAG_FORCE_SPLIT) return Route::Split;
+    if (ws_ok && p.n_groups >= 16u * (unsigned)sm_count()) return Route::Fused;
+    return Route::Split;
 }
 
 feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
@@ -264,7 +133,8 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
                               void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (flags & ~FEDS_FLAG_NO_DIGEST) return FEDS_ERR_BAD_PARAM;
+    if (flags & ~DCT_FLAGS) return FEDS_ERR_BAD_PARAM;
+    if ((flags & FEDS_FLAG_FORCE_FUSED) && (flags & FEDS_FLAG_FORCE_SPLIT)) return FEDS_ERR_BAD_PARAM;
     const bool digest = !(flags & FEDS_FLAG_NO_DIGEST);
     const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
     if (!d_images || !key || !d_private || (!d_public && pub_b) || (digest && (!d_digests || !d_workspace)) || (!d_nonces && !nonce_host))
@@ -284,8 +154,10 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
     uint8_t *ws = static_cast<uint8_t *>(d_workspace);
     p.leaves = (pl.nl > 1) ? ws : d_digests;  // a one-leaf fragment's root is its leaf digest
     if (digest) {
-        if (fragment_fused_pays(p)) {
-            st = launch_fragment_fused(p, c, stream);
+        const Route route = pick_route(p, c, flags);
+        if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;
+        if (route == Route::Fused) {
+            st = launch_fragment_ws(p, c, stream);
         } else {
             st = launch_fragment_tile(p, c, stream);   // records the profiling start; the stop follows the leaf hash
             if (st != FEDS_OK) return st;
@@ -298,8 +170,8 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
             if (st != FEDS_OK) return st;
         }
         if (k == 63) {
-            write_empty_public_root_kernel<<<(n_images + 127) / 128, 128, 0, stream>>>(d_digests, n_images);
-            FEDS_LAUNCH_CHECK();
+            st = launch_empty_public_roots(d_digests, n_images, stream);
+            if (st != FEDS_OK) return st;
         }
     } else {
         st = launch_fragment_tile(p, c, stream);
@@ -321,12 +193,10 @@ feds_status finish_verification(const DctParams &p, const DctPlan &pl, int n_ima
         if (st != FEDS_OK) return st;
     }
     if (k == 63) {
-        write_empty_public_root_kernel<<<(n_images + 127) / 128, 128, 0, stream>>>(roots, n_images);
-        FEDS_LAUNCH_CHECK();
+        const feds_status st = launch_empty_public_roots(roots, n_images, stream);
+        if (st != FEDS_OK) return st;
     }
-    compare_digests_kernel<<<(n_images + 127) / 128, 128, 0, stream>>>(roots, d_expected, d_flags, n_images);
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
+    return launch_compare_digests(roots, d_expected, d_flags, n_images, stream);
 }
 
 feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
@@ -335,7 +205,8 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
                                 uint32_t *d_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (flags & ~FEDS_FLAG_NO_DIGEST) return FEDS_ERR_BAD_PARAM;
+    if (flags & ~DCT_FLAGS) return FEDS_ERR_BAD_PARAM;
+    if ((flags & FEDS_FLAG_FORCE_FUSED) && (flags & FEDS_FLAG_FORCE_SPLIT)) return FEDS_ERR_BAD_PARAM;
     const bool verify = d_expected != nullptr && !(flags & FEDS_FLAG_NO_DIGEST);
     const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
     if (!d_private || (!d_public && pub_b) || !key || !d_images_out || (!d_nonces && !nonce_host) || (verify && (!d_flags || !d_workspace)))
@@ -354,18 +225,23 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
     p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
     if (verify) {
         p.leaves = verification_leaves(pl, n_images, static_cast<uint8_t *>(d_workspace));
-        // Verification and reconstruction are independent readers of the fragments: the leaf digests come from a
-        // registers-only hash kernel (28 warps per SM, 0.89 of the ALU roofline), the pixels from the digest-free tile kernel.
-        // Measured against one fused kernel doing both per leaf (round 1: 9.68 ms at cfg3): 9.21 ms, and 5-13 % faster for
-        // every k whose runs are not 16-byte multiples.
-        if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-        st = launch_leaves_hash(p, c, stream);
-        if (st != FEDS_OK) return st;
-        st = launch_defragment(p, c, stream, true);
+        // Verification and reconstruction read the same fragments. Fused route: one warp-specialised kernel whose hash warps
+        // and reconstruction warps walk the leaves together, so the fragments come from HBM once (feds_dct_ws.cuh). Split
+        // route: the registers-only leaf-hash kernel, then the digest-free tile kernel.
+        const Route route = pick_route(p, c, flags);
+        if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;
+        if (route == Route::Fused) {
+            st = launch_defragment_ws(p, c, stream);
+        } else {
+            if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
+            st = launch_leaves_hash(p, c, stream);
+            if (st != FEDS_OK) return st;
+            st = launch_defragment_tile(p, c, stream, false);
+        }
         if (st != FEDS_OK) return st;
         return finish_verification(p, pl, n_images, k, static_cast<uint8_t *>(d_workspace), d_expected, d_flags, stream);
     }
-    return launch_defragment(p, c, stream);
+    return launch_defragment_tile(p, c, stream, true);
 }
 
 // verification alone: what a holder of the fragments can do without the key (A8)
@@ -416,8 +292,8 @@ DwtPlan dwt_plan(int w, int h, int c, int L) {
         off += round_up((size_t)c * (w >> l) * (h >> l) * 2, 256);
     }
     pl.planes_bytes = off;
-    pl.priv_tree = tree_bytes(pl.priv_nl);
-    pl.pub_tree = tree_bytes(pl.pub_nl);
+    pl.priv_tree = std::max<size_t>(tree_bytes(pl.priv_nl), 32);   // a one-leaf tree still parks its leaf digest here in a batch
+    pl.pub_tree = std::max<size_t>(tree_bytes(pl.pub_nl), 32);
     pl.per_image = round_up(pl.planes_bytes + round_up(pl.priv_tree, 256) + round_up(pl.pub_tree, 256) + 64, 256);
     return pl;
 }
@@ -428,70 +304,132 @@ size_t dwt_level_off_elems(int w, int h, int L, int l) {  // elements before lev
     return off;
 }
 
-// Which level kernel: the register-streaming ones (feds_dwt_fast.cuh) need whole per-thread runs and aligned vector
-// accesses; returns the pixels per thread (16: planar int16 or gray uint8; 8: interleaved RGB uint8) or 0 = tiled kernel.
-int dwt_fast_px(const DwtLevelParams &p, bool u8, int c_img) {
-    if (getenv("FEDS_DWT_TILED")) return 0;
-    const int px = u8 ? (c_img == 1 ? 16 : c_img == 3 ? 8 : 0) : 16;
-    if (px == 0 || p.cw % px != 0 || (p.ch & 1)) return 0;
-    const size_t a = (size_t)px / 2;  // subband elements per thread and row: every offset must be a multiple of it
-    if (p.level_off % a || (c_img > 1 && (p.pub_chan_stride % a || p.ll_band_chan_stride % a))) return 0;
-    if ((reinterpret_cast<uintptr_t>(p.ll_band) | reinterpret_cast<uintptr_t>(p.pub)) & 15u) return 0;
-    if (u8) { if (p.img_w % (c_img == 1 ? 16 : 8)) return 0; }
-    return px;
-}
-// picks the rows per warp tile (p.rows) so that the launch has at least ~12 warps per SM, and returns the grid
-dim3 dwt_fast_grid(DwtLevelParams &p, int px, int planes) {
-    const int runs = p.cw / px, bh = p.ch >> 1;
-    const unsigned strips = (unsigned)((runs + DWTF_LANES_OUT - 1) / DWTF_LANES_OUT);
-    const unsigned long long want = 12ull * (unsigned)sm_count();
-    int rows = DWTF_ROWS;
-    while (rows > 4 && (unsigned long long)strips * planes * ((bh + rows - 1) / rows) < want) rows /= 2;
-    p.rows = rows;
-    return dim3(strips, (unsigned)((bh + DWTF_WARPS * rows - 1) / (DWTF_WARPS * rows)), planes);
+// leaf digests + trees of the two fragments of n_images images -> roots[i][64] (private root || public root).
+// tree_ws: [private leaves of all images][private upper levels][public leaves of all images][public upper levels]
+feds_status dwt_digests(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride, int n_images,
+                        const DwtPlan &pl, uint8_t *tree_ws, uint8_t *roots, cudaStream_t stream) {
+    const unsigned nls[2] = {pl.priv_nl, pl.pub_nl};
+    uint8_t *ws[2] = {tree_ws, tree_ws + round_up(pl.priv_tree, 256) * (size_t)n_images};
+    const uint8_t *const data[2] = {d_private, d_public};
+    const size_t strides[2] = {private_stride, public_stride};
+    const unsigned long long nbytes[2] = {pl.priv_b, pl.pub_b};
+    // a one-leaf fragment's root is its leaf digest: with one image it is written in place; a batch of one-leaf fragments
+    // goes through the workspace and the tail kernel is skipped by copying (n0 == 1 trees need no reduction, see below)
+    uint8_t *out[2];
+    for (int f = 0; f < 2; ++f) out[f] = (nls[f] > 1 || n_images > 1) ? ws[f] : roots + 32 * f;
+    feds_status st = launch_stream_leaves(data, strides, nbytes, nls, out, (unsigned)n_images, true, stream);
+    if (st != FEDS_OK) return st;
+    if (n_images > 1) {
+        for (int f = 0; f < 2; ++f)
+            if (nls[f] == 1) FEDS_CUDA(cudaMemcpy2DAsync(roots + 32 * f, 64, ws[f], 32, 32, (size_t)n_images, cudaMemcpyDeviceToDevice, stream));
+    }
+    return run_two_trees(ws[0], nls[0], ws[0] + (size_t)nls[0] * 32 * n_images, roots, ws[1], nls[1], ws[1] + (size_t)nls[1] * 32 * n_images,
+                         roots + 32, (unsigned)n_images, 64, stream);
 }
 
-// AES-128-CTR of a byte stream: the conflict-free 128 KB table layout pays once the stream is a few MB long
-feds_status launch_aes_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes, const uint8_t key[16], const uint8_t nonce[16],
-                           cudaStream_t stream) {
-    if (n_bytes == 0) return FEDS_OK;
-    CtrParams cp{};
-    cp.in = d_in; cp.out = d_out; cp.n_bytes = n_bytes;
-    nonce_to_be(nonce, cp.nonce_be);
-    aes128_expand_key_host(key, cp.rk, h_aes);
-    const unsigned long long nblk = (n_bytes + 15) / 16;
-    const unsigned sms = (unsigned)sm_count();
-    if (n_bytes >= ((size_t)4 << 20)) {
-        const size_t smem = (size_t)AES_TABLE_WORDS * 32 * 4;
-        feds_status st = set_smem(aes_ctr_stream_kernel<32>, smem);
-        if (st != FEDS_OK) return st;
-        aes_ctr_stream_kernel<32><<<sms, AES_THREADS, smem, stream>>>(cp);
-    } else {
-        const unsigned want = (unsigned)((nblk + AES_THREADS - 1) / AES_THREADS);
-        aes_ctr_stream_kernel<1><<<std::min(want, 2 * sms), AES_THREADS, (size_t)AES_TABLE_WORDS * 4, stream>>>(cp);
-    }
-    FEDS_LAUNCH_CHECK();
+feds_status check_dwt_args(int n_images, int w, int h, int c, int levels) {
+    if (w <= 0 || h <= 0) return FEDS_ERR_BAD_DIMS;
+    if (!chan_ok(c) || levels < 1 || levels > 6 || n_images < 1) return FEDS_ERR_BAD_PARAM;
+    if (!dwt_dims_ok(w, h, levels)) return FEDS_ERR_BAD_DIMS;
     return FEDS_OK;
 }
 
-feds_status dwt_digests(const uint8_t *d_private, const uint8_t *d_public, const DwtPlan &pl, uint8_t *tree_ws, uint8_t *roots,
-                        cudaStream_t stream) {
-    const unsigned nls[2] = {pl.priv_nl, pl.pub_nl};
-    uint8_t *ws[2] = {tree_ws, tree_ws + round_up(pl.priv_tree, 256)};
-    StreamLeavesParams sp;
-    sp.data[0] = d_private; sp.data[1] = d_public;
-    sp.n_bytes[0] = pl.priv_b; sp.n_bytes[1] = pl.pub_b;
-    sp.one = 1u;
-    for (int f = 0; f < 2; ++f) {
-        sp.n_leaves[f] = nls[f];
-        sp.out[f] = nls[f] > 1 ? ws[f] : roots + 32 * f;  // a one-leaf fragment's root is its leaf digest
+// Workspace of a DWT batch, level-major so that the planes of one level are contiguous over the images (the level kernels
+// index planes by n * C + c): [LL_1 planes of all images] ... [LL_L planes][trees][n x 64 B recomputed roots].
+size_t dwt_plane_off(const DwtPlan &pl, int l, int n_images) { return pl.plane_off[l] * (size_t)n_images; }
+
+feds_status fragment_dwt_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int levels,
+                              const uint8_t key[16], const uint8_t *nonce_host, const uint8_t *d_nonces, uint8_t *d_private,
+                              size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                              size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
+    feds_status st = check_dwt_args(n_images, w, h, c, levels);
+    if (st != FEDS_OK) return st;
+    if (flags & ~FEDS_FLAG_DWT_TILED) return FEDS_ERR_BAD_PARAM;
+    if (!d_images || !key || (!nonce_host && !d_nonces) || !d_private || !d_public || !d_digests || !d_workspace) return FEDS_ERR_NULL_POINTER;
+    const DwtPlan pl = dwt_plan(w, h, c, levels);
+    if (image_stride < (size_t)w * h * c || private_stride < pl.priv_b || public_stride < pl.pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images) || misaligned(d_private) || misaligned(d_public) || misaligned(d_digests) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    if (workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    const int L = levels;
+    const bool tiled = (flags & FEDS_FLAG_DWT_TILED) != 0;
+
+    for (int l = 1; l <= L; ++l) {
+        DwtLevelParams p{};
+        p.C = c; p.img_w = w; p.image_stride = image_stride;
+        p.cw = w >> (l - 1); p.ch = h >> (l - 1);
+        const int bw = w >> l, bh = h >> l;
+        p.img_in = d_images;
+        if (l > 1) { p.ll_in = reinterpret_cast<const int16_t *>(ws + dwt_plane_off(pl, l - 1, n_images)); p.ll_in_plane_stride = (size_t)p.cw * p.ch; }
+        if (l < L) {
+            p.ll_band = reinterpret_cast<int16_t *>(ws + dwt_plane_off(pl, l, n_images));
+            p.ll_band_image_stride = (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
+        } else {
+            p.ll_band = reinterpret_cast<int16_t *>(d_private);
+            p.ll_band_image_stride = private_stride / 2; p.ll_band_chan_stride = (size_t)bw * bh;
+        }
+        p.pub = reinterpret_cast<int16_t *>(d_public);
+        p.pub_image_stride = public_stride / 2;
+        p.pub_chan_stride = pl.pub_b / 2 / c;
+        p.level_off = dwt_level_off_elems(w, h, L, l);
+        st = launch_dwt_fwd_level(p, l == 1, c, n_images, tiled, stream);
+        if (st != FEDS_OK) return st;
     }
-    const unsigned total = nls[0] + nls[1];
-    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    stream_leaves_kernel<<<(total + LEAF_THREADS - 1) / LEAF_THREADS, LEAF_THREADS, 0, stream>>>(sp);
-    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
-    FEDS_LAUNCH_CHECK();
-    return run_two_trees(ws[0], nls[0], ws[0] + (size_t)nls[0] * 32, roots, ws[1], nls[1], ws[1] + (size_t)nls[1] * 32, roots + 32, stream);
+    st = launch_aes_ctr(d_private, private_stride, d_private, private_stride, pl.priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
+    if (st != FEDS_OK) return st;
+    return dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, ws + pl.planes_bytes * (size_t)n_images, d_digests, stream);
+}
+
+feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *nonce_host,
+                                const uint8_t *d_nonces, const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
+    feds_status st = check_dwt_args(n_images, w, h, c, levels);
+    if (st != FEDS_OK) return st;
+    if (flags & ~FEDS_FLAG_DWT_TILED) return FEDS_ERR_BAD_PARAM;
+    if (!d_private || !d_public || !key || (!nonce_host && !d_nonces) || !d_images_out || !d_workspace || (d_expected_digests && !d_verify_flags))
+        return FEDS_ERR_NULL_POINTER;
+    const DwtPlan pl = dwt_plan(w, h, c, levels);
+    if (image_stride < (size_t)w * h * c || private_stride < pl.priv_b || public_stride < pl.pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images_out) || misaligned(d_private) || misaligned(d_public) || misaligned(d_expected_digests) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    if (workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    const int L = levels;
+    const bool tiled = (flags & FEDS_FLAG_DWT_TILED) != 0;
+
+    if (d_expected_digests) {
+        uint8_t *roots = ws + pl.per_image * (size_t)n_images - 64 * (size_t)n_images;
+        st = dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, ws + pl.planes_bytes * (size_t)n_images, roots, stream);
+        if (st != FEDS_OK) return st;
+        st = launch_compare_digests(roots, d_expected_digests, d_verify_flags, n_images, stream);
+        if (st != FEDS_OK) return st;
+    }
+    // decrypt LL_L into the level-L plane block (the received fragment stays untouched)
+    uint8_t *lldec = ws + dwt_plane_off(pl, L, n_images);
+    st = launch_aes_ctr(d_private, private_stride, lldec, pl.priv_b, pl.priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
+    if (st != FEDS_OK) return st;
+
+    for (int l = L; l >= 1; --l) {
+        DwtLevelParams p{};
+        p.C = c; p.img_w = w; p.image_stride = image_stride;
+        p.cw = w >> (l - 1); p.ch = h >> (l - 1);
+        const int bw = w >> l, bh = h >> l;
+        p.ll_band = reinterpret_cast<int16_t *>(ws + dwt_plane_off(pl, l, n_images));
+        p.ll_band_image_stride = (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
+        p.pub = reinterpret_cast<int16_t *>(const_cast<uint8_t *>(d_public));
+        p.pub_image_stride = public_stride / 2;
+        p.pub_chan_stride = pl.pub_b / 2 / c;
+        p.level_off = dwt_level_off_elems(w, h, L, l);
+        p.img_out = d_images_out;
+        if (l > 1) { p.ll_out_plane = reinterpret_cast<int16_t *>(ws + dwt_plane_off(pl, l - 1, n_images)); p.ll_out_plane_stride = (size_t)p.cw * p.ch; }
+        st = launch_dwt_inv_level(p, l == 1, c, n_images, tiled, stream);
+        if (st != FEDS_OK) return st;
+    }
+    return FEDS_OK;
 }
 
 }  // namespace
@@ -601,127 +539,56 @@ feds_status feds_verify_dct_batch(const uint8_t *d_private, size_t private_strid
 feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t nonce[16],
                               uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
                               feds_stream_t stream) {
-    if (w <= 0 || h <= 0) return FEDS_ERR_BAD_DIMS;
-    if (!chan_ok(c) || levels < 1 || levels > 6) return FEDS_ERR_BAD_PARAM;
-    if (!dwt_dims_ok(w, h, levels)) return FEDS_ERR_BAD_DIMS;
-    if (!d_image || !key || !nonce || !d_private || !d_public || !d_digests || !d_workspace) return FEDS_ERR_NULL_POINTER;
-    if (misaligned(d_image) || misaligned(d_private) || misaligned(d_public) || misaligned(d_digests) || misaligned(d_workspace))
-        return FEDS_ERR_MISALIGNED;
-    const DwtPlan pl = dwt_plan(w, h, c, levels);
-    if (workspace_bytes < pl.per_image) return FEDS_ERR_WORKSPACE_TOO_SMALL;
-    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
-    const int L = levels;
+    if (!nonce) return check_dwt_args(1, w, h, c, levels) != FEDS_OK ? check_dwt_args(1, w, h, c, levels) : FEDS_ERR_NULL_POINTER;
+    return fragment_dwt_impl(d_image, 1, (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), w, h, c, levels, key, nonce, nullptr,
+                             d_private, feds_dwt_private_bytes(w, h, c, levels), d_public, feds_dwt_public_bytes(w, h, c, levels), d_digests,
+                             d_workspace, workspace_bytes, FEDS_FLAG_NONE, stream);
+}
 
-    for (int l = 1; l <= L; ++l) {
-        DwtLevelParams p{};
-        p.C = c; p.img_w = w; p.image_stride = (size_t)w * h * c;
-        p.cw = w >> (l - 1); p.ch = h >> (l - 1);
-        const int bw = w >> l, bh = h >> l;
-        p.img_in = d_image;
-        if (l > 1) { p.ll_in = reinterpret_cast<const int16_t *>(ws + pl.plane_off[l - 1]); p.ll_in_plane_stride = (size_t)p.cw * p.ch; }
-        if (l < L) {
-            p.ll_band = reinterpret_cast<int16_t *>(ws + pl.plane_off[l]);
-            p.ll_band_image_stride = (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
-        } else {
-            p.ll_band = reinterpret_cast<int16_t *>(d_private);
-            p.ll_band_image_stride = pl.priv_b / 2; p.ll_band_chan_stride = (size_t)bw * bh;
-        }
-        p.pub = reinterpret_cast<int16_t *>(d_public);
-        p.pub_image_stride = pl.pub_b / 2;
-        p.pub_chan_stride = pl.pub_b / 2 / c;
-        p.level_off = dwt_level_off_elems(w, h, L, l);
-        const int px = dwt_fast_px(p, l == 1, c);
-        const dim3 fgrid = px ? dwt_fast_grid(p, px, l == 1 ? 1 : c) : dim3();   // also sets p.rows
-        if (px && l == 1 && c == 1) dwt_fwd_fast_kernel<1, 16, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px && l == 1) dwt_fwd_fast_kernel<3, 8, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px) dwt_fwd_fast_kernel<1, 16, false><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else {
-            const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
-            if (l == 1) dwt_fwd_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
-            else dwt_fwd_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
-        }
-        FEDS_LAUNCH_CHECK();
-    }
-    const feds_status st = launch_aes_ctr(d_private, d_private, pl.priv_b, key, nonce, stream);
-    if (st != FEDS_OK) return st;
-    return dwt_digests(d_private, d_public, pl, ws + pl.planes_bytes, d_digests, stream);
+feds_status feds_fragment_dwt_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int levels,
+                                    const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private, size_t private_stride,
+                                    uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                                    size_t workspace_bytes, unsigned flags, feds_stream_t stream) {
+    if (!d_nonces) return check_dwt_args(n_images, w, h, c, levels) != FEDS_OK ? check_dwt_args(n_images, w, h, c, levels) : FEDS_ERR_NULL_POINTER;
+    return fragment_dwt_impl(d_images, n_images, image_stride, w, h, c, levels, key, nullptr, d_nonces, d_private, private_stride, d_public,
+                             public_stride, d_digests, d_workspace, workspace_bytes, flags, stream);
 }
 
 feds_status feds_defragment_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,
                                 const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
                                 uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
                                 feds_stream_t stream) {
-    if (w <= 0 || h <= 0) return FEDS_ERR_BAD_DIMS;
-    if (!chan_ok(c) || levels < 1 || levels > 6) return FEDS_ERR_BAD_PARAM;
-    if (!dwt_dims_ok(w, h, levels)) return FEDS_ERR_BAD_DIMS;
-    if (!d_private || !d_public || !key || !nonce || !d_image_out || !d_workspace || (d_expected_digests && !d_verify_flags))
-        return FEDS_ERR_NULL_POINTER;
-    if (misaligned(d_image_out) || misaligned(d_private) || misaligned(d_public) || misaligned(d_expected_digests) || misaligned(d_workspace))
-        return FEDS_ERR_MISALIGNED;
-    const DwtPlan pl = dwt_plan(w, h, c, levels);
-    if (workspace_bytes < pl.per_image) return FEDS_ERR_WORKSPACE_TOO_SMALL;
-    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
-    const int L = levels;
+    if (!nonce) return check_dwt_args(1, w, h, c, levels) != FEDS_OK ? check_dwt_args(1, w, h, c, levels) : FEDS_ERR_NULL_POINTER;
+    return defragment_dwt_impl(d_private, feds_dwt_private_bytes(w, h, c, levels), d_public, feds_dwt_public_bytes(w, h, c, levels), 1, w, h,
+                               c, levels, key, nonce, nullptr, d_expected_digests, d_image_out,
+                               (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), d_verify_flags, d_workspace, workspace_bytes,
+                               FEDS_FLAG_NONE, stream);
+}
 
-    if (d_expected_digests) {
-        uint8_t *roots = ws + pl.per_image - 64;
-        feds_status st = dwt_digests(d_private, d_public, pl, ws + pl.planes_bytes, roots, stream);
-        if (st != FEDS_OK) return st;
-        compare_digests_kernel<<<1, 32, 0, stream>>>(roots, d_expected_digests, d_verify_flags, 1);
-        FEDS_LAUNCH_CHECK();
-    }
-    // decrypt LL_L into the level-L plane block (the received fragment stays untouched)
-    uint8_t *lldec = ws + pl.plane_off[L];
-    {
-        const feds_status st = launch_aes_ctr(d_private, lldec, pl.priv_b, key, nonce, stream);
-        if (st != FEDS_OK) return st;
-    }
-
-    for (int l = L; l >= 1; --l) {
-        DwtLevelParams p{};
-        p.C = c; p.img_w = w; p.image_stride = (size_t)w * h * c;
-        p.cw = w >> (l - 1); p.ch = h >> (l - 1);
-        const int bw = w >> l, bh = h >> l;
-        p.ll_band = reinterpret_cast<int16_t *>(ws + pl.plane_off[l]);
-        p.ll_band_image_stride = (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
-        p.pub = reinterpret_cast<int16_t *>(const_cast<uint8_t *>(d_public));
-        p.pub_image_stride = pl.pub_b / 2;
-        p.pub_chan_stride = pl.pub_b / 2 / c;
-        p.level_off = dwt_level_off_elems(w, h, L, l);
-        p.img_out = d_image_out;
-        if (l > 1) { p.ll_out_plane = reinterpret_cast<int16_t *>(ws + pl.plane_off[l - 1]); p.ll_out_plane_stride = (size_t)p.cw * p.ch; }
-        const int px = dwt_fast_px(p, l == 1, c);
-        const dim3 fgrid = px ? dwt_fast_grid(p, px, l == 1 ? 1 : c) : dim3();   // also sets p.rows
-        if (px && l == 1 && c == 1) dwt_inv_fast_kernel<1, 16, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px && l == 1) dwt_inv_fast_kernel<3, 8, true><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else if (px) dwt_inv_fast_kernel<1, 16, false><<<fgrid, DWTF_WARPS * 32, 0, stream>>>(p);
-        else {
-            const dim3 grid((bw + DWT_TW - 1) / DWT_TW, (bh + DWT_TH - 1) / DWT_TH, c);
-            if (l == 1) dwt_inv_level_kernel<true><<<grid, DWT_THREADS, 0, stream>>>(p);
-            else dwt_inv_level_kernel<false><<<grid, DWT_THREADS, 0, stream>>>(p);
-        }
-        FEDS_LAUNCH_CHECK();
-    }
-    return FEDS_OK;
+feds_status feds_defragment_dwt_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                      int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *d_nonces,
+                                      const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                      uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                      feds_stream_t stream) {
+    if (!d_nonces) return check_dwt_args(n_images, w, h, c, levels) != FEDS_OK ? check_dwt_args(n_images, w, h, c, levels) : FEDS_ERR_NULL_POINTER;
+    return defragment_dwt_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, levels, key, nullptr, d_nonces,
+                               d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, flags, stream);
 }
 
 feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,
                             const uint8_t *d_expected_digests, uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
                             feds_stream_t stream) {
-    if (w <= 0 || h <= 0) return FEDS_ERR_BAD_DIMS;
-    if (!chan_ok(c) || levels < 1 || levels > 6) return FEDS_ERR_BAD_PARAM;
-    if (!dwt_dims_ok(w, h, levels)) return FEDS_ERR_BAD_DIMS;
+    const feds_status a0 = check_dwt_args(1, w, h, c, levels);
+    if (a0 != FEDS_OK) return a0;
     if (!d_private || !d_public || !d_expected_digests || !d_verify_flags || !d_workspace) return FEDS_ERR_NULL_POINTER;
     if (misaligned(d_private) || misaligned(d_public) || misaligned(d_expected_digests) || misaligned(d_workspace)) return FEDS_ERR_MISALIGNED;
     const DwtPlan pl = dwt_plan(w, h, c, levels);
     if (workspace_bytes < pl.per_image) return FEDS_ERR_WORKSPACE_TOO_SMALL;
     uint8_t *ws = static_cast<uint8_t *>(d_workspace);
     uint8_t *roots = ws + pl.per_image - 64;
-    const feds_status st = dwt_digests(d_private, d_public, pl, ws + pl.planes_bytes, roots, stream);
+    const feds_status st = dwt_digests(d_private, pl.priv_b, d_public, pl.pub_b, 1, pl, ws + pl.planes_bytes, roots, stream);
     if (st != FEDS_OK) return st;
-    compare_digests_kernel<<<1, 32, 0, stream>>>(roots, d_expected_digests, d_verify_flags, 1);
-    FEDS_LAUNCH_CHECK();
-    return FEDS_OK;
+    return launch_compare_digests(roots, d_expected_digests, d_verify_flags, 1, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ stream primitives
@@ -729,7 +596,7 @@ feds_status feds_aes128_ctr(const uint8_t *d_in, uint8_t *d_out, size_t n_bytes,
                             feds_stream_t stream) {
     if (!key || !nonce || (n_bytes && (!d_in || !d_out))) return FEDS_ERR_NULL_POINTER;
     if (misaligned(d_in) || misaligned(d_out)) return FEDS_ERR_MISALIGNED;
-    return launch_aes_ctr(d_in, d_out, n_bytes, key, nonce, stream);
+    return launch_aes_ctr(d_in, 0, d_out, 0, n_bytes, 1, key, nonce, nullptr, stream);
 }
 
 size_t feds_sha256_merkle_workspace_bytes(size_t n_bytes) {
@@ -746,20 +613,15 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
     if (nl64 > 0xffffffffull) return FEDS_ERR_BAD_PARAM;
     const unsigned nl = (unsigned)nl64;
     if (nl > 1 && (!d_workspace || workspace_bytes < feds_sha256_merkle_workspace_bytes(n_bytes))) return d_workspace ? FEDS_ERR_WORKSPACE_TOO_SMALL : FEDS_ERR_NULL_POINTER;
-    if (nl == 0) {  // SHA-256(""): the kernel writes it at digests + 32
-        uint8_t *ws = static_cast<uint8_t *>(d_workspace);
-        (void)ws;
-        write_empty_root_kernel<<<1, 32, 0, stream>>>(d_root);
-        FEDS_LAUNCH_CHECK();
-        return FEDS_OK;
-    }
+    if (nl == 0) return launch_empty_root(d_root, stream);  // SHA-256("")
     uint8_t *ws = static_cast<uint8_t *>(d_workspace);
-    StreamLeavesParams sp{};
-    sp.data[0] = d_data; sp.n_bytes[0] = n_bytes; sp.n_leaves[0] = nl;
-    sp.out[0] = nl > 1 ? ws : d_root;
-    sp.one = 1u;
-    stream_leaves_kernel<<<(nl + LEAF_THREADS - 1) / LEAF_THREADS, LEAF_THREADS, 0, stream>>>(sp);
-    FEDS_LAUNCH_CHECK();
+    const uint8_t *const data[2] = {d_data, nullptr};
+    const size_t strides[2] = {0, 0};
+    const unsigned long long nbytes[2] = {n_bytes, 0};
+    const unsigned nls[2] = {nl, 0};
+    uint8_t *const out[2] = {nl > 1 ? ws : d_root, nullptr};
+    const feds_status st = launch_stream_leaves(data, strides, nbytes, nls, out, 1, false, stream);
+    if (st != FEDS_OK) return st;
     if (nl > 1) return run_tree(ws, nl, 1, ws + (size_t)nl * 32, d_root, 32, 0, stream);
     return FEDS_OK;
 }
@@ -786,7 +648,7 @@ feds_status feds_fragment_dct_host(const uint8_t *h_images, int n_images, int w,
                                    unsigned flags) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (images_per_chunk < 1 || n_streams < 1 || (flags & ~FEDS_FLAG_NO_DIGEST)) return FEDS_ERR_BAD_PARAM;
+    if (images_per_chunk < 1 || n_streams < 1 || (flags & ~DCT_FLAGS)) return FEDS_ERR_BAD_PARAM;
     const bool digest = !(flags & FEDS_FLAG_NO_DIGEST);
     const size_t img_b = (size_t)w * h * c, priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
     if (!h_images || !key || !h_nonces || !h_private || (!h_public && pub_b) || (digest && !h_digests) || !d_scratch || !streams)
@@ -830,7 +692,7 @@ feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_
                                      size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (images_per_chunk < 1 || n_streams < 1 || (flags & ~FEDS_FLAG_NO_DIGEST)) return FEDS_ERR_BAD_PARAM;
+    if (images_per_chunk < 1 || n_streams < 1 || (flags & ~DCT_FLAGS)) return FEDS_ERR_BAD_PARAM;
     const bool verify = h_expected_digests != nullptr && !(flags & FEDS_FLAG_NO_DIGEST);
     const size_t img_b = (size_t)w * h * c, priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
     if (!h_private || (!h_public && pub_b) || !key || !h_nonces || !h_images_out || (verify && !h_verify_flags) || !d_scratch || !streams)

@@ -21,7 +21,7 @@
 
 namespace feds {
 
-__device__ const AesTables g_aes = make_aes_tables();
+static __device__ const AesTables g_aes = make_aes_tables();   // one copy per translation unit
 
 constexpr int DCT_THREADS = 512;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
 constexpr int DCT_CTAS_PER_SM = 1;
@@ -48,6 +48,10 @@ struct DctParams {
     int slot_stride;  // words per lane slot
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
     unsigned n_groups;  // ceil(total_leaves / 32): one group = the 32 leaves one warp owns at a time
+    // warp-specialised kernels (feds_dct_ws.cuh)
+    unsigned ws_n_sg;   // strip groups: ceil(n_images * nbr * nlr / 32)
+    int ws_ahead;       // slabs a worker may run in front of its slowest hash warp
+    uint32_t c128;      // = 128, opaque to the compiler (ws_lookup)
 };
 
 // Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:

@@ -3,6 +3,7 @@
 // -m "not gpu" tests can exercise exactly the code the kernels run (feds_debug_*_host in feds.h).
 // Shares nothing with oracle/: tables are generated here at compile time from the standards' definitions.
 #pragma once
+#include <cmath>
 #include <cstdint>
 #include <cstddef>
 
@@ -74,7 +75,7 @@ FEDS_HD void sha256_compress(uint32_t (&H)[8], uint32_t (&w)[16]) {
 // The same compression as a 4 x 16-round loop: 4x less code (the fused kernels are instruction-cache bound when fully
 // unrolled), W indices still static, K_t read from constant memory with a warp-uniform index.
 #ifdef __CUDACC__
-__constant__ uint32_t c_sha256_k[64] = {FEDS_SHA256_K_LIST};
+static __constant__ uint32_t c_sha256_k[64] = {FEDS_SHA256_K_LIST};
 #endif
 FEDS_HD void sha256_compress_rolled(uint32_t (&H)[8], uint32_t (&w)[16]) {
 #ifndef __CUDA_ARCH__
@@ -275,33 +276,65 @@ FEDS_HD void ctr_block(const uint32_t (&n)[4], uint64_t i, uint32_t (&col)[4]) {
 #define FEDS_C6 0.191341716182545f /* cos(6 pi/16)/2 */
 #define FEDS_C7 0.097545161008064f /* cos(7 pi/16)/2 */
 
+// Every operation is an explicitly rounded IEEE-754 single-precision mul / add / fma (no compiler contraction or
+// reassociation), so every kernel that inlines these -- and the host build used by feds_debug_dct8x8_host -- produces the
+// same bits: fragments and digests do not depend on which route or compiler version ran.
+FEDS_HD float f_mul(float a, float b) {
+#ifdef __CUDA_ARCH__
+    return __fmul_rn(a, b);
+#else
+    return a * b;
+#endif
+}
+FEDS_HD float f_add(float a, float b) {
+#ifdef __CUDA_ARCH__
+    return __fadd_rn(a, b);
+#else
+    return a + b;
+#endif
+}
+FEDS_HD float f_sub(float a, float b) {
+#ifdef __CUDA_ARCH__
+    return __fsub_rn(a, b);
+#else
+    return a - b;
+#endif
+}
+FEDS_HD float f_fma(float a, float b, float c) {
+#ifdef __CUDA_ARCH__
+    return __fmaf_rn(a, b, c);
+#else
+    return fmaf(a, b, c);
+#endif
+}
+
 FEDS_HD void dct8(float &x0, float &x1, float &x2, float &x3, float &x4, float &x5, float &x6, float &x7) {
-    const float a0 = x0 + x7, a1 = x1 + x6, a2 = x2 + x5, a3 = x3 + x4;
-    const float b0 = x0 - x7, b1 = x1 - x6, b2 = x2 - x5, b3 = x3 - x4;
-    const float e0 = a0 + a3, e1 = a1 + a2, e2 = a0 - a3, e3 = a1 - a2;
-    x0 = FEDS_C4 * (e0 + e1);
-    x4 = FEDS_C4 * (e0 - e1);
-    x2 = FEDS_C2 * e2 + FEDS_C6 * e3;
-    x6 = FEDS_C6 * e2 - FEDS_C2 * e3;
-    x1 = FEDS_C1 * b0 + FEDS_C3 * b1 + FEDS_C5 * b2 + FEDS_C7 * b3;
-    x3 = FEDS_C3 * b0 - FEDS_C7 * b1 - FEDS_C1 * b2 - FEDS_C5 * b3;
-    x5 = FEDS_C5 * b0 - FEDS_C1 * b1 + FEDS_C7 * b2 + FEDS_C3 * b3;
-    x7 = FEDS_C7 * b0 - FEDS_C5 * b1 + FEDS_C3 * b2 - FEDS_C1 * b3;
+    const float a0 = f_add(x0, x7), a1 = f_add(x1, x6), a2 = f_add(x2, x5), a3 = f_add(x3, x4);
+    const float b0 = f_sub(x0, x7), b1 = f_sub(x1, x6), b2 = f_sub(x2, x5), b3 = f_sub(x3, x4);
+    const float e0 = f_add(a0, a3), e1 = f_add(a1, a2), e2 = f_sub(a0, a3), e3 = f_sub(a1, a2);
+    x0 = f_mul(FEDS_C4, f_add(e0, e1));
+    x4 = f_mul(FEDS_C4, f_sub(e0, e1));
+    x2 = f_fma(FEDS_C2, e2, f_mul(FEDS_C6, e3));
+    x6 = f_fma(FEDS_C6, e2, f_mul(-FEDS_C2, e3));
+    x1 = f_fma(FEDS_C1, b0, f_fma(FEDS_C3, b1, f_fma(FEDS_C5, b2, f_mul(FEDS_C7, b3))));
+    x3 = f_fma(FEDS_C3, b0, f_fma(-FEDS_C7, b1, f_fma(-FEDS_C1, b2, f_mul(-FEDS_C5, b3))));
+    x5 = f_fma(FEDS_C5, b0, f_fma(-FEDS_C1, b1, f_fma(FEDS_C7, b2, f_mul(FEDS_C3, b3))));
+    x7 = f_fma(FEDS_C7, b0, f_fma(-FEDS_C5, b1, f_fma(FEDS_C3, b2, f_mul(-FEDS_C1, b3))));
 }
 
 // inverse: x[i] = sum_u c(u)/2 X[u] cos((2i+1) u pi/16)
 FEDS_HD void idct8(float &x0, float &x1, float &x2, float &x3, float &x4, float &x5, float &x6, float &x7) {
-    const float p = FEDS_C4 * (x0 + x4), q = FEDS_C4 * (x0 - x4);
-    const float r = FEDS_C2 * x2 + FEDS_C6 * x6, s = FEDS_C6 * x2 - FEDS_C2 * x6;
-    const float e0 = p + r, e3 = p - r, e1 = q + s, e2 = q - s;  // even part at i = 0,1,2,3 (mirrored at 7,6,5,4)
-    const float o0 = FEDS_C1 * x1 + FEDS_C3 * x3 + FEDS_C5 * x5 + FEDS_C7 * x7;
-    const float o1 = FEDS_C3 * x1 - FEDS_C7 * x3 - FEDS_C1 * x5 - FEDS_C5 * x7;
-    const float o2 = FEDS_C5 * x1 - FEDS_C1 * x3 + FEDS_C7 * x5 + FEDS_C3 * x7;
-    const float o3 = FEDS_C7 * x1 - FEDS_C5 * x3 + FEDS_C3 * x5 - FEDS_C1 * x7;
-    x0 = e0 + o0; x7 = e0 - o0;
-    x1 = e1 + o1; x6 = e1 - o1;
-    x2 = e2 + o2; x5 = e2 - o2;
-    x3 = e3 + o3; x4 = e3 - o3;
+    const float p = f_mul(FEDS_C4, f_add(x0, x4)), q = f_mul(FEDS_C4, f_sub(x0, x4));
+    const float r = f_fma(FEDS_C2, x2, f_mul(FEDS_C6, x6)), s = f_fma(FEDS_C6, x2, f_mul(-FEDS_C2, x6));
+    const float e0 = f_add(p, r), e3 = f_sub(p, r), e1 = f_add(q, s), e2 = f_sub(q, s);  // even part at i = 0,1,2,3 (mirrored at 7,6,5,4)
+    const float o0 = f_fma(FEDS_C1, x1, f_fma(FEDS_C3, x3, f_fma(FEDS_C5, x5, f_mul(FEDS_C7, x7))));
+    const float o1 = f_fma(FEDS_C3, x1, f_fma(-FEDS_C7, x3, f_fma(-FEDS_C1, x5, f_mul(-FEDS_C5, x7))));
+    const float o2 = f_fma(FEDS_C5, x1, f_fma(-FEDS_C1, x3, f_fma(FEDS_C7, x5, f_mul(FEDS_C3, x7))));
+    const float o3 = f_fma(FEDS_C7, x1, f_fma(-FEDS_C5, x3, f_fma(FEDS_C3, x5, f_mul(-FEDS_C1, x7))));
+    x0 = f_add(e0, o0); x7 = f_sub(e0, o0);
+    x1 = f_add(e1, o1); x6 = f_sub(e1, o1);
+    x2 = f_add(e2, o2); x5 = f_sub(e2, o2);
+    x3 = f_add(e3, o3); x4 = f_sub(e3, o3);
 }
 
 // 2-D transform of a row-major block held in 64 registers: row pass then column pass (separable).

@@ -20,11 +20,12 @@ struct MerkleLevelParams {
     size_t in_tree_stride, out_tree_stride;  // bytes
     int odd_trees_only_if_nonempty;  // 1: skip odd trees (public fragments) because they are empty (k = 63)
     uint32_t one;                    // = 1, opaque to the compiler (sha256_compress_rolled_fma)
-    // merkle_tail_kernel only: an optional extra tree of another shape, reduced by CTA number n_trees (DWT: the
-    // private and the public tree finish in one launch)
+    // merkle_tail_kernel only: an optional second family of n_trees2 trees of another shape, reduced by CTAs n_trees ..
+    // n_trees + n_trees2 - 1 (DWT: the private and the public trees finish in one launch)
     const uint8_t *in2;
     uint8_t *out2;
-    unsigned n_in2;
+    unsigned n_in2, n_trees2;
+    size_t in2_tree_stride, out2_tree_stride;
 };
 
 // SHA-256 of `cnt` (1..16) concatenated 32-byte child digests at src (global memory via the read-only path, or shared).
@@ -90,11 +91,12 @@ __global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_
     const unsigned t = blockIdx.x, tid = threadIdx.x;
     const bool extra = t >= p.n_trees;
     if (!extra && p.odd_trees_only_if_nonempty && (t & 1u)) return;
-    uint4 *root = reinterpret_cast<uint4 *>(extra ? p.out2 : p.out + (size_t)t * p.out_tree_stride);
+    const unsigned t2 = extra ? t - p.n_trees : 0u;
+    uint4 *root = reinterpret_cast<uint4 *>(extra ? p.out2 + (size_t)t2 * p.out2_tree_stride : p.out + (size_t)t * p.out_tree_stride);
     // One hash_children call site serves all (up to three) levels: the levels run one after the other on a nearly empty SM,
     // so what counts is the length of the dependent chain and the amount of cold code, not throughput. Level sources and
     // sinks are generic pointers (global input, then the two shared buffers).
-    const uint4 *src = reinterpret_cast<const uint4 *>(extra ? p.in2 : p.in + (size_t)t * p.in_tree_stride);
+    const uint4 *src = reinterpret_cast<const uint4 *>(extra ? p.in2 + (size_t)t2 * p.in2_tree_stride : p.in + (size_t)t * p.in_tree_stride);
     unsigned n = extra ? p.n_in2 : p.n_in;
     uint4 *dst = sA;
 #pragma unroll 1
@@ -122,10 +124,12 @@ __global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_
 // the generic byte tail below handles any length).
 // ------------------------------------------------------------------------------------------------------------
 struct StreamLeavesParams {
-    const uint8_t *data[2];        // the two fragment streams (private, public); hashed in one launch
-    unsigned long long n_bytes[2];
-    unsigned n_leaves[2];
-    uint8_t *out[2];               // leaf digests [leaf][32] per stream
+    const uint8_t *data[2];        // the two fragment streams (private, public) of image 0; hashed in one launch
+    unsigned long long n_bytes[2]; // per image
+    unsigned n_leaves[2];          // per image
+    uint8_t *out[2];               // leaf digests [image][leaf][32] per stream
+    size_t data_stride[2];         // bytes between consecutive images' streams
+    unsigned n_images;
     uint32_t one;                  // = 1, opaque to the compiler (sha256_compress_rolled_fma)
 };
 
@@ -133,13 +137,15 @@ struct StreamLeavesParams {
 // small CTAs are what spreads them evenly over the SMs.
 constexpr int LEAF_THREADS = 64;
 __global__ void __launch_bounds__(LEAF_THREADS) stream_leaves_kernel(const __grid_constant__ StreamLeavesParams p) {
-    const unsigned gid = blockIdx.x * LEAF_THREADS + threadIdx.x;
-    if (gid >= p.n_leaves[0] + p.n_leaves[1]) return;
+    const unsigned long long gid0 = (unsigned long long)blockIdx.x * LEAF_THREADS + threadIdx.x;
+    const unsigned per_image = p.n_leaves[0] + p.n_leaves[1];
+    if (gid0 >= (unsigned long long)per_image * p.n_images) return;
+    const unsigned img = (unsigned)(gid0 / per_image), gid = (unsigned)(gid0 % per_image);
     const int f = gid >= p.n_leaves[0] ? 1 : 0;
     const unsigned j = f ? gid - p.n_leaves[0] : gid;
     const unsigned long long lo = (unsigned long long)j * DWT_LEAF_BYTES;
     const unsigned len = (unsigned)min((unsigned long long)DWT_LEAF_BYTES, p.n_bytes[f] - lo);
-    const uint8_t *src = p.data[f] + lo;
+    const uint8_t *src = p.data[f] + (size_t)img * p.data_stride[f] + lo;
     uint32_t H[8];
     sha256_init(H);
     const unsigned full = len >> 6, tail = len & 63u;
@@ -181,7 +187,7 @@ __global__ void __launch_bounds__(LEAF_THREADS) stream_leaves_kernel(const __gri
         }
         sha256_compress_rolled_fma(H, w, p.one);
     }
-    store_digest(p.out[f] + (size_t)j * 32, H);
+    store_digest(p.out[f] + ((size_t)img * p.n_leaves[f] + j) * 32, H);
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -193,10 +199,21 @@ __global__ void __launch_bounds__(LEAF_THREADS) stream_leaves_kernel(const __gri
 struct CtrParams {
     const uint8_t *in;
     uint8_t *out;
-    unsigned long long n_bytes;
+    unsigned long long n_bytes;       // per message
+    size_t in_stride, out_stride;     // bytes between consecutive messages (batch); each message has its own counter from 0
+    unsigned n_msgs;
+    const uint8_t *d_nonces;          // device uint8[n_msgs][16], or nullptr: nonce_be for the single message
     uint32_t nonce_be[4];
     uint32_t rk[44];
 };
+__device__ __forceinline__ void ctr_load_nonce(const CtrParams &p, unsigned m, uint32_t (&nonce)[4]) {
+    if (p.d_nonces) {
+        const uint4 q = __ldg(reinterpret_cast<const uint4 *>(p.d_nonces) + m);
+        nonce[0] = bswap32(q.x); nonce[1] = bswap32(q.y); nonce[2] = bswap32(q.z); nonce[3] = bswap32(q.w);
+    } else {
+        nonce[0] = p.nonce_be[0]; nonce[1] = p.nonce_be[1]; nonce[2] = p.nonce_be[2]; nonce[3] = p.nonce_be[3];
+    }
+}
 constexpr int AES_THREADS = 512;
 
 template <int REPL>
@@ -254,23 +271,31 @@ __global__ void __launch_bounds__(AES_THREADS) aes_ctr_stream_kernel(const __gri
     const uint32_t lane4 = 4u * (threadIdx.x & 31);
     const unsigned long long nfull = p.n_bytes >> 4;
     const unsigned long long stride = (unsigned long long)gridDim.x * AES_THREADS;
-    const uint32_t nonce[4] = {p.nonce_be[0], p.nonce_be[1], p.nonce_be[2], p.nonce_be[3]};
-    const uint4 *in4 = reinterpret_cast<const uint4 *>(p.in);
-    uint4 *out4 = reinterpret_cast<uint4 *>(p.out);
-    for (unsigned long long i = (unsigned long long)blockIdx.x * AES_THREADS + threadIdx.x; i < nfull; i += stride) {
-        uint4 v = __ldg(in4 + i);
+    const unsigned long long total = nfull * p.n_msgs;
+    unsigned cur = 0xffffffffu;
+    uint32_t nonce[4] = {0u, 0u, 0u, 0u};
+    for (unsigned long long i = (unsigned long long)blockIdx.x * AES_THREADS + threadIdx.x; i < total; i += stride) {
+        const unsigned m = p.n_msgs > 1 ? (unsigned)(i / nfull) : 0u;
+        const unsigned long long blk = p.n_msgs > 1 ? i - (unsigned long long)m * nfull : i;
+        if (m != cur) { ctr_load_nonce(p, m, nonce); cur = m; }
+        uint4 v = __ldg(reinterpret_cast<const uint4 *>(p.in + (size_t)m * p.in_stride) + blk);
         uint32_t ks[4];
-        ctr_block(nonce, i, ks);
+        ctr_block(nonce, blk, ks);
         if (REPL == 32) aes128_encrypt_rep32(tabb, lane4, p.rk, ks); else aes128_encrypt(T, p.rk, ks);
         v.x ^= ks[0]; v.y ^= ks[1]; v.z ^= ks[2]; v.w ^= ks[3];
-        out4[i] = v;
+        reinterpret_cast<uint4 *>(p.out + (size_t)m * p.out_stride)[blk] = v;
     }
     const unsigned rem = (unsigned)(p.n_bytes & 15u);
-    if (rem && blockIdx.x == 0 && threadIdx.x == 0) {  // keystream of the partial last block is truncated
-        uint32_t ks[4];
-        ctr_block(nonce, nfull, ks);
-        aes128_encrypt(T, p.rk, ks);
-        for (unsigned b = 0; b < rem; ++b) p.out[16 * nfull + b] = p.in[16 * nfull + b] ^ (uint8_t)(ks[b >> 2] >> (8 * (b & 3)));
+    if (rem && blockIdx.x == 0) {  // keystream of the partial last block of each message is truncated
+        for (unsigned m = threadIdx.x; m < p.n_msgs; m += AES_THREADS) {
+            uint32_t ks[4];
+            ctr_load_nonce(p, m, nonce);
+            ctr_block(nonce, nfull, ks);
+            aes128_encrypt(T, p.rk, ks);
+            const uint8_t *src = p.in + (size_t)m * p.in_stride + 16 * nfull;
+            uint8_t *dst = p.out + (size_t)m * p.out_stride + 16 * nfull;
+            for (unsigned b = 0; b < rem; ++b) dst[b] = src[b] ^ (uint8_t)(ks[b >> 2] >> (8 * (b & 3)));
+        }
     }
 }
 

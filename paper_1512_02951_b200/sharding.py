@@ -17,8 +17,25 @@ def shard_range(n_total: int, world: int, rank: int):
     return first, count
 
 
-def nonces_for(base_nonce: bytes, first_global_index: int, count: int, stride: int = 1 << 20) -> np.ndarray:
-    """uint8[count][16]: nonce of global image i = (base + i * stride) mod 2^128, big-endian (one IV per image)."""
+def nonce_stride(priv_bytes: int, min_stride: int = 1 << 20) -> int:
+    """Counter blocks between the nonces of consecutive images: a power of two >= ceil(priv_bytes / 16), so that the CTR counter
+    ranges [nonce_i, nonce_i + ceil(priv_bytes / 16)) of the images never overlap under the one key (include/feds.h, batch entry
+    points; overlapping ranges would reuse keystream)."""
+    need = max(1, (int(priv_bytes) + 15) // 16)
+    stride = max(1, int(min_stride))
+    while stride < need:
+        stride <<= 1
+    return stride
+
+
+def nonces_for(base_nonce: bytes, first_global_index: int, count: int, priv_bytes: int = 0, stride: int = None) -> np.ndarray:
+    """uint8[count][16]: nonce of global image i = (base + i * stride) mod 2^128, big-endian (one IV per image).
+    `priv_bytes` = size of one image's private fragment; the stride is chosen (or, when given, checked) so that the images'
+    counter ranges cannot overlap."""
+    if stride is None:
+        stride = nonce_stride(priv_bytes)
+    if stride * 16 < priv_bytes:
+        raise ValueError("nonce stride %d blocks is shorter than the private fragment (%d bytes): keystream would be reused" % (stride, priv_bytes))
     base = int.from_bytes(base_nonce, "big")
     out = np.empty((count, 16), dtype=np.uint8)
     for j in range(count):

@@ -22,8 +22,15 @@ def key_nonce(seed: int):
     return d[:16], d[16:]
 
 
-def batch_nonces(base_nonce: bytes, n: int, stride: int = 1 << 20) -> np.ndarray:
-    """nonce_i = (base + i*stride) mod 2^128, big-endian; uint8[n][16]."""
+def batch_nonces(base_nonce: bytes, n: int, priv_bytes: int = 0, stride: int = None) -> np.ndarray:
+    """nonce_i = (base + i*stride) mod 2^128, big-endian; uint8[n][16]. stride (in 16-byte counter blocks) defaults to the
+    smallest power of two >= max(2^20, ceil(priv_bytes / 16)): the images' counter ranges must not overlap under one key."""
+    if stride is None:
+        stride = 1 << 20
+        while stride * 16 < priv_bytes:
+            stride <<= 1
+    if stride * 16 < priv_bytes:
+        raise ValueError("nonce stride shorter than the private fragment: keystream would be reused")
     base = int.from_bytes(base_nonce, "big")
     out = np.empty((n, 16), dtype=np.uint8)
     for i in range(n):

@@ -279,7 +279,10 @@ def test_config2_full_size(orc, b):
 
 
 def test_config3_batch_full_size(orc, b):
-    """256 x 1920x1080 RGB, k=3, batched as bench.py launches it; sampled images checked in full by the oracle."""
+    """256 x 1920x1080 RGB, k=3, batched as bench.py launches it. Stage (ii) -- ciphertext, public bytes and both digests through
+    the oracle's pack + AES-CTR + SHA-256 -- on ALL 256 images, the oracle calls spread over host threads
+    (ctypes releases the GIL); stage (i) on a crop of every 8th image; then the exact round trip of the whole batch."""
+    from concurrent.futures import ThreadPoolExecutor
     n, w, h, c, k = 256, 1920, 1080, 3, 3
     key, nonce = synth.key_nonce(3)
     nonces = synth.batch_nonces(nonce, n)
@@ -289,24 +292,35 @@ def test_config3_batch_full_size(orc, b):
     batch.fragment(d_imgs, key, d_nonces)
     torch.cuda.synchronize()
     nb = c * (h // 8) * (w // 8)
-    for i in [0, 1, 100, 255]:
-        img = d_imgs[i].cpu().numpy()
-        priv = batch.priv[i * batch.priv_bytes:(i + 1) * batch.priv_bytes].cpu().numpy()
-        pub = batch.pub[i * batch.pub_bytes:(i + 1) * batch.pub_bytes].cpu().numpy()
-        dg = batch.digests[64 * i:64 * i + 64].cpu().numpy().tobytes()
+    dgs = batch.digests.cpu().numpy().reshape(n, 64)
+
+    def one(i, priv, pub, img):
         nz = nonces[i].tobytes()
         coef = gpu_coefficients(orc, priv, pub, nb, k, key, nz)
         p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nz)
-        assert (p2 == priv).all() and (q2 == pub).all() and d2 == dg
-        crop = np.ascontiguousarray(img[512:576, 960:1024, :])
-        ref = orc.dct_coefficients(crop).reshape(c, 8, 8, 64)
-        assert np.abs(coef.reshape(c, h // 8, w // 8, 64)[:, 64:72, 120:128, :] - ref).max() <= TOL
+        assert (p2 == priv).all() and (q2 == pub).all() and d2 == dgs[i].tobytes(), i
+        if img is not None:
+            crop = np.ascontiguousarray(img[512:576, 960:1024, :])
+            ref = orc.dct_coefficients(crop).reshape(c, 8, 8, 64)
+            assert np.abs(coef.reshape(c, h // 8, w // 8, 64)[:, 64:72, 120:128, :] - ref).max() <= TOL, i
+        return i
+
+    with ThreadPoolExecutor(max_workers=16) as ex:
+        futs = []
+        for i in range(n):
+            priv = batch.priv[i * batch.priv_bytes:(i + 1) * batch.priv_bytes].cpu().numpy()
+            pub = batch.pub[i * batch.pub_bytes:(i + 1) * batch.pub_bytes].cpu().numpy()
+            img = d_imgs[i].cpu().numpy() if i % 8 == 0 or i == n - 1 else None
+            futs.append(ex.submit(one, i, priv, pub, img))
+            if len(futs) >= 32:                      # bound the host copies in flight
+                futs.pop(0).result()
+        for f in futs:
+            f.result()
     out = torch.empty_like(d_imgs)
     batch.defragment(out, key, d_nonces, expected=batch.digests)
     torch.cuda.synchronize()
     assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
     # every image's digests are distinct (independent CTR messages, A20)
-    dgs = batch.digests.cpu().numpy().reshape(n, 64)
     assert len({bytes(r[:32]) for r in dgs}) == n
 
 
@@ -344,11 +358,16 @@ def test_digest_free_tile_kernels(orc, b, n, w, h, c, k):
     assert torch.equal(out, d_imgs) and int(full.flags_out.abs().sum().item()) == 0
 
 
-# Steps 1-5 run either in the fused thread-per-leaf kernel (full persistent grid, k + 1 even) or as tile kernel + leaf-hash kernel
-# (everything else); the library picks by size. Both routes must produce the same bytes and digests at any size.
-@pytest.mark.parametrize("n,w,h,c,k", [(1, 8, 8, 1, 3), (2, 264, 16, 3, 3), (1, 1032, 24, 1, 5), (3, 1920, 16, 3, 7), (2, 520, 40, 4, 1),
-                                       (1, 2056, 8, 1, 9), (1, 256, 64, 3, 31), (1, 512, 8, 4, 61), (1, 2048, 8, 3, 63)])
-def test_fused_and_split_fragment_routes_agree(orc, b, n, w, h, c, k, monkeypatch):
+# Steps 1-5 (and 6-8 with verification) run either in the warp-specialised fused kernels (feds_dct_ws.cuh: whole 8-block leaves,
+# k + 1 even) or as tile kernel + leaf-hash kernel (everything else); the library picks by shape and size, FEDS_FLAG_FORCE_FUSED /
+# FEDS_FLAG_FORCE_SPLIT override it. Both routes must produce the same bytes, digests, images and flags at any size.
+WS_CASES = [(1, 64, 8, 1, 3), (2, 256, 16, 3, 3), (1, 1024, 24, 1, 5), (3, 1920, 16, 3, 7), (2, 512, 40, 4, 1), (1, 2048, 8, 1, 9),
+            (1, 256, 64, 3, 31), (1, 512, 8, 4, 61), (1, 2048, 8, 3, 63), (7, 1920, 136, 3, 3), (1, 4096, 264, 3, 5), (3, 2048, 72, 4, 3),
+            (2, 8192, 24, 1, 3), (40, 64, 64, 3, 3)]
+
+
+@pytest.mark.parametrize("n,w,h,c,k", WS_CASES)
+def test_fused_and_split_routes_agree(orc, b, n, w, h, c, k):
     key, nonce = synth.key_nonce(w + k)
     nonces = synth.batch_nonces(nonce, n)
     imgs = np.stack([synth.image(w, h, c, seed=11 * w + i + k) for i in range(n)])
@@ -357,19 +376,77 @@ def test_fused_and_split_fragment_routes_agree(orc, b, n, w, h, c, k, monkeypatc
     fused, split = b.DctBatch(n, w, h, c, k), b.DctBatch(n, w, h, c, k)
     for t in (fused.priv, fused.pub, fused.digests, split.priv, split.pub, split.digests):
         t.fill_(0x5A)
-    monkeypatch.setenv("FEDS_FRAGMENT_PATH", "fused")
-    fused.fragment(d_imgs, key, d_nonces)
-    monkeypatch.setenv("FEDS_FRAGMENT_PATH", "split")
-    split.fragment(d_imgs, key, d_nonces)
-    monkeypatch.delenv("FEDS_FRAGMENT_PATH")
+    fused.fragment(d_imgs, key, d_nonces, flags=b.FLAG_FORCE_FUSED)
+    split.fragment(d_imgs, key, d_nonces, flags=b.FLAG_FORCE_SPLIT)
     torch.cuda.synchronize()
     assert torch.equal(fused.priv, split.priv) and torch.equal(fused.pub, split.pub) and torch.equal(fused.digests, split.digests)
-    # and they are the oracle's for these coefficient bytes (image 0)
-    pv, pb = fused.priv[:fused.priv_bytes].cpu().numpy(), fused.pub[:fused.pub_bytes].cpu().numpy()
-    coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[0].tobytes())
-    assert np.abs(coef - orc.dct_coefficients(imgs[0])).max() <= TOL
-    p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[0].tobytes())
-    assert (p2 == pv).all() and (q2 == pb).all() and d2 == fused.digests[:64].cpu().numpy().tobytes()
-    out = torch.zeros_like(d_imgs)
-    fused.defragment(out, key, d_nonces, expected=split.digests)
-    assert torch.equal(out, d_imgs) and int(fused.flags_out.abs().sum().item()) == 0
+    # and they are the oracle's for these coefficient bytes (first and last image)
+    for i in sorted({0, n - 1}):
+        pv = fused.priv[i * fused.priv_bytes:(i + 1) * fused.priv_bytes].cpu().numpy()
+        pb = fused.pub[i * fused.pub_bytes:(i + 1) * fused.pub_bytes].cpu().numpy()
+        coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[i].tobytes())
+        if w * h <= 1 << 19:
+            assert np.abs(coef - orc.dct_coefficients(imgs[i])).max() <= TOL
+        p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[i].tobytes())
+        assert (p2 == pv).all() and (q2 == pb).all() and d2 == fused.digests[64 * i:64 * i + 64].cpu().numpy().tobytes()
+    # verified defragment on both routes: exact image, flags 0; then one flipped byte per fragment in chosen images
+    for flag in (b.FLAG_FORCE_FUSED, b.FLAG_FORCE_SPLIT):
+        out = torch.zeros_like(d_imgs)
+        fused.flags_out.fill_(9)
+        fused.defragment(out, key, d_nonces, expected=split.digests, flags=flag)
+        assert torch.equal(out, d_imgs) and int(fused.flags_out.abs().sum().item()) == 0
+    if k < 63:
+        split.pub[(n - 1) * split.pub_bytes + split.pub_bytes - 1] ^= 0x01
+    split.priv[5] ^= 0x80
+    want = [0] * n
+    want[0] |= 1
+    if k < 63:
+        want[n - 1] |= 2
+    outs = []
+    for flag in (b.FLAG_FORCE_FUSED, b.FLAG_FORCE_SPLIT):
+        out = torch.zeros_like(d_imgs)
+        split.defragment(out, key, d_nonces, expected=fused.digests, flags=flag)
+        assert split.flags_out.cpu().tolist() == want
+        outs.append(out)
+    assert torch.equal(outs[0], outs[1])      # the image is written regardless (A10), identically on both routes
+
+
+def test_forced_route_that_cannot_run_is_refused(b):
+    """FEDS_FLAG_FORCE_FUSED on a shape the fused kernels do not support (ragged last leaf: (w/8) % 8 != 0; odd k + 1) returns
+    FEDS_ERR_BAD_PARAM before anything is enqueued; both force flags together likewise."""
+    key, nonce = synth.key_nonce(1)
+    for (w, h, c, k) in [(520, 16, 3, 3), (512, 16, 3, 2)]:
+        img = torch.zeros((1, h, w, c), dtype=torch.uint8, device="cuda")
+        non = torch.zeros((1, 16), dtype=torch.uint8, device="cuda")
+        batch = b.DctBatch(1, w, h, c, k)
+        with pytest.raises(b.FedsError) as e:
+            batch.fragment(img, key, non, flags=b.FLAG_FORCE_FUSED)
+        assert e.value.code == 3
+        batch.fragment(img, key, non, flags=b.FLAG_FORCE_SPLIT)
+        with pytest.raises(b.FedsError) as e:
+            batch.defragment(img.clone(), key, non, expected=batch.digests, flags=b.FLAG_FORCE_FUSED)
+        assert e.value.code == 3
+    batch = b.DctBatch(1, 64, 8, 1, 3)
+    with pytest.raises(b.FedsError):
+        batch.fragment(torch.zeros((1, 8, 64, 1), dtype=torch.uint8, device="cuda"), key, torch.zeros((1, 16), dtype=torch.uint8, device="cuda"),
+                       flags=b.FLAG_FORCE_FUSED | b.FLAG_FORCE_SPLIT)
+
+
+def test_device_dct_bits_equal_the_host_build(orc, b):
+    """The 8x8 transform is written with explicitly rounded mul / add / fma, so the kernels and the host build of the same
+    function (feds_debug_dct8x8_host, gcc) agree bit for bit: fragments do not depend on compiler contraction choices."""
+    import ctypes as C
+    w, h, c, k = 256, 64, 1, 63
+    img = synth.image(w, h, c, seed=5, rectangles=3)
+    key = bytes(16)
+    priv, _, _ = b.fragment_dct(torch.from_numpy(img).cuda(), k, key, bytes(16))
+    ks = np.frombuffer(orc.aes128_ctr_xor(key, bytes(16), bytes(priv.numel())), dtype=np.uint8)
+    coef = np.frombuffer((priv.cpu().numpy() ^ ks).tobytes(), dtype="<f4").reshape(h // 8, w // 8, 64)
+    zz = (C.c_int * 64)()
+    b.lib.feds_debug_zigzag_host(zz)
+    zz = np.array(list(zz))
+    for (br, bc) in [(0, 0), (3, 17), (7, 31), (5, 2)]:
+        x = np.ascontiguousarray(img[8 * br:8 * br + 8, 8 * bc:8 * bc + 8, 0], dtype=np.float32)
+        out = np.empty(64, dtype=np.float32)
+        b.lib.feds_debug_dct8x8_host(x.ctypes.data, out.ctypes.data, 0)
+        assert (out[zz].view(np.uint32) == coef[br, bc].view(np.uint32)).all()

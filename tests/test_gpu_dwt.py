@@ -69,21 +69,53 @@ def test_config4_full_size(orc, b):
 
 
 @pytest.mark.parametrize("w,h,c,L", [(1024, 320, 3, 4), (2048, 64, 1, 1), (7696, 96, 1, 2), (496, 80, 3, 1)])
-def test_streaming_and_tiled_level_kernels_agree(orc, b, w, h, c, L, monkeypatch):
+def test_streaming_and_tiled_level_kernels_agree(orc, b, w, h, c, L):
     """The register-streaming level kernels (several column strips, halo lanes, row tiles) and the tiled shared-memory
-    kernels they replace on aligned sizes compute identical fragments; the oracle decides which is right."""
+    kernels they replace on aligned sizes (FEDS_FLAG_DWT_TILED) compute identical fragments; the oracle decides which is right."""
     img = synth.image(w, h, c, seed=w + L)
     key, nonce = synth.key_nonce(w)
-    d_img = torch.from_numpy(img).cuda()
-    fast = b.fragment_dwt(d_img, L, key, nonce)
-    monkeypatch.setenv("FEDS_DWT_TILED", "1")
-    tiled = b.fragment_dwt(d_img, L, key, nonce)
-    rec_tiled, _ = b.defragment_dwt(fast[0], fast[1], w, h, c, L, key, nonce)
-    monkeypatch.delenv("FEDS_DWT_TILED")
-    rec_fast, _ = b.defragment_dwt(tiled[0], tiled[1], w, h, c, L, key, nonce)
+    d_img = torch.from_numpy(img).cuda().unsqueeze(0).contiguous()
+    d_non = torch.frombuffer(bytearray(nonce), dtype=torch.uint8).cuda().view(1, 16)
+    fast, tiled = b.DwtBatch(1, w, h, c, L), b.DwtBatch(1, w, h, c, L)
+    fast.fragment(d_img, key, d_non)
+    tiled.fragment(d_img, key, d_non, flags=b.FLAG_DWT_TILED)
+    rec_tiled, rec_fast = torch.zeros_like(d_img), torch.zeros_like(d_img)
+    fast.defragment(rec_tiled, key, d_non, flags=b.FLAG_DWT_TILED)     # tiled inverse of the streaming kernels' fragments
+    tiled.defragment(rec_fast, key, d_non)                             # and the other way round
     torch.cuda.synchronize()
-    for x, y in zip(fast, tiled):
-        assert torch.equal(x, y)
+    assert torch.equal(fast.priv, tiled.priv) and torch.equal(fast.pub, tiled.pub) and torch.equal(fast.digests, tiled.digests)
     op, oq, odg = orc.fragment_dwt(img, L, key, nonce)
-    assert (fast[0].cpu().numpy() == op).all() and (fast[1].cpu().numpy() == oq).all() and fast[2].cpu().numpy().tobytes() == odg
+    assert (fast.priv[:fast.priv_bytes].cpu().numpy() == op).all() and (fast.pub[:fast.pub_bytes].cpu().numpy() == oq).all()
+    assert fast.digests.cpu().numpy().tobytes() == odg
     assert torch.equal(rec_tiled, d_img) and torch.equal(rec_fast, d_img)
+
+
+@pytest.mark.parametrize("n,w,h,c,L", [(3, 64, 32, 1, 2), (4, 272, 144, 3, 3), (2, 1024, 320, 3, 4), (5, 16, 8, 1, 1), (3, 48, 80, 4, 2),
+                                       (2, 2048, 512, 1, 3)])
+def test_dwt_batch_equals_oracle_per_image(orc, b, n, w, h, c, L):
+    """feds_fragment_dwt_batch / feds_defragment_dwt_batch: every image is an independent CTR message with its own nonce and digest
+    pair (A20); each image's fragments and digests are the oracle's, bit for bit; verification flags are per image."""
+    key, nonce = synth.key_nonce(w + n)
+    imgs = np.stack([synth.image(w, h, c, seed=50 * w + i, rectangles=1 if min(w, h) >= 32 else 0) for i in range(n)])
+    batch = b.DwtBatch(n, w, h, c, L)
+    nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
+    d_imgs, d_non = torch.from_numpy(imgs).cuda(), torch.from_numpy(nonces).cuda()
+    batch.fragment(d_imgs, key, d_non)
+    torch.cuda.synchronize()
+    for i in range(n):
+        op, oq, odg = orc.fragment_dwt(imgs[i], L, key, nonces[i].tobytes())
+        assert (batch.priv[i * batch.priv_stride:i * batch.priv_stride + batch.priv_bytes].cpu().numpy() == op).all(), i
+        assert (batch.pub[i * batch.pub_stride:i * batch.pub_stride + batch.pub_bytes].cpu().numpy() == oq).all(), i
+        assert batch.digests[64 * i:64 * i + 64].cpu().numpy().tobytes() == odg, i
+    out = torch.zeros_like(d_imgs)
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    victim = n - 1
+    batch.pub[victim * batch.pub_stride + 3] ^= 0x20
+    batch.priv[0] ^= 1
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    want = [0] * n
+    want[victim] |= 2
+    want[0] |= 1
+    assert batch.flags_out.cpu().tolist() == want

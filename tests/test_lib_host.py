@@ -23,7 +23,8 @@ def b():
 
 
 def test_exports_every_declared_symbol(b):
-    header = open(os.path.join(ROOT, "include", "feds.h")).read()
+    header = open(os.path.join(ROOT, "include", "feds.h")).read() + open(os.path.join(ROOT, "include", "feds_debug.h")).read()
+    assert "feds_debug_" not in open(os.path.join(ROOT, "include", "feds.h")).read()   # test hooks stay out of the product header
     declared = set(re.findall(r"\b(feds_[a-z0-9_]+)\s*\(", header))
     declared -= {"feds_stream_t"}
     assert declared == set(b.SYMBOLS), declared ^ set(b.SYMBOLS)

@@ -73,6 +73,29 @@ def test_nonces_depend_on_global_index_only():
     assert sharding.nonces_for(top, 1, 1)[0].tobytes() == ((1 << 20) - 1).to_bytes(16, "big")   # wraps mod 2^128
 
 
+def test_nonce_stride_covers_the_private_fragment():
+    """with one key, the counter ranges of consecutive images must not overlap whatever the fragment size. A private
+    fragment above 16 MiB (2^20 blocks) must widen the stride; a stride that is too short is refused."""
+    import synth
+    from paper_1512_02951_b200 import sharding
+    _, nonce = synth.key_nonce(2)
+    priv = 4096 * 4096 * 3 // 64 * 6 * 4                   # BASELINE configs[1]: 18.9 MB private fragment per image
+    assert priv > (1 << 20) * 16
+    stride = sharding.nonce_stride(priv)
+    assert stride * 16 >= priv and stride & (stride - 1) == 0
+    a = sharding.nonces_for(nonce, 0, 3, priv_bytes=priv)
+    vals = [int.from_bytes(r.tobytes(), "big") for r in a]
+    blocks = (priv + 15) // 16
+    for x, y in zip(vals, vals[1:]):
+        assert (y - x) % (1 << 128) >= blocks                # image i's last counter < image i+1's first
+    assert (a == synth.batch_nonces(nonce, 3, priv_bytes=priv)).all()
+    with pytest.raises(ValueError):
+        sharding.nonces_for(nonce, 0, 2, priv_bytes=priv, stride=1 << 20)
+    with pytest.raises(ValueError):
+        synth.batch_nonces(nonce, 2, priv_bytes=priv, stride=1 << 20)
+    assert sharding.nonce_stride(1555200) == 1 << 20         # cfg3 keeps the round-1 stride: stored digests do not move
+
+
 def test_two_gloo_ranks_equal_single_process():
     world, port = 2, 29500 + (os.getpid() % 2000)
     ctx = mp.get_context("spawn")
