@@ -50,6 +50,7 @@ typedef enum {
 #define FEDS_FLAG_FORCE_FUSED 2u /* DCT with digests: the warp-specialised fused kernel (needs (w/8) % 8 == 0 and k + 1 even) */
 #define FEDS_FLAG_FORCE_SPLIT 4u /* DCT with digests: digest-free tile kernel + leaf-hash kernel */
 #define FEDS_FLAG_DWT_TILED 8u   /* DWT: the tiled shared-memory level kernels instead of the register-streaming ones */
+#define FEDS_FLAG_GENERIC_TILES 16u /* DCT: the generic tile kernels (any w) even where the bulk-copy (TMA) tile kernels apply (w % 32 == 0) */
 
 const char *feds_status_string(feds_status s);
 int feds_last_cuda_error(void); /* cudaError_t of the most recent FEDS_ERR_CUDA on this thread, else 0 */

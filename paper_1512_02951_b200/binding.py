@@ -16,6 +16,7 @@ FLAG_NO_DIGEST = 1
 FLAG_FORCE_FUSED = 2
 FLAG_FORCE_SPLIT = 4
 FLAG_DWT_TILED = 8
+FLAG_GENERIC_TILES = 16
 
 STATUS = {0: "FEDS_OK", 1: "FEDS_ERR_NULL_POINTER", 2: "FEDS_ERR_BAD_DIMS", 3: "FEDS_ERR_BAD_PARAM",
           4: "FEDS_ERR_WORKSPACE_TOO_SMALL", 5: "FEDS_ERR_CUDA", 6: "FEDS_ERR_MISALIGNED"}

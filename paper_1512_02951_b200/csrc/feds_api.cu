@@ -117,7 +117,7 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
 // Which route fragments with digests. The warp-specialised fused kernel (feds_dct_ws.cuh) needs whole 8-block leaves and
 // 8/16-byte runs, and pays once its persistent grid is full; everything else runs as the digest-free tile kernel followed
 // by the leaf-hash kernel over what it wrote.
-constexpr unsigned DCT_FLAGS = FEDS_FLAG_NO_DIGEST | FEDS_FLAG_FORCE_FUSED | FEDS_FLAG_FORCE_SPLIT;
+constexpr unsigned DCT_FLAGS = FEDS_FLAG_NO_DIGEST | FEDS_FLAG_FORCE_FUSED | FEDS_FLAG_FORCE_SPLIT | FEDS_FLAG_GENERIC_TILES;
 enum class Route { Fused, Split, Unsupported };
 Route pick_route(const DctParams &p, int c, unsigned flags) {
     const bool ws_ok = dct_ws_supported(p, c);
@@ -148,6 +148,7 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
 
     DctParams p;
     fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, digest);
+    p.generic_tiles = (flags & FEDS_FLAG_GENERIC_TILES) ? 1 : 0;
     p.images = d_images; p.image_stride = image_stride;
     p.priv = d_private; p.priv_stride = private_stride;
     p.pub = d_public; p.pub_stride = public_stride;
@@ -220,6 +221,7 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
 
     DctParams p;
     fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, verify);
+    p.generic_tiles = (flags & FEDS_FLAG_GENERIC_TILES) ? 1 : 0;
     p.images_out = d_images_out; p.image_stride = image_stride;
     p.priv = const_cast<uint8_t *>(d_private); p.priv_stride = private_stride;
     p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
@@ -409,8 +411,10 @@ feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride,
         if (st != FEDS_OK) return st;
     }
     // decrypt LL_L into the level-L plane block (the received fragment stays untouched)
+    // (image stride rounded up to 16 bytes: the CTR kernel moves 128-bit words; the plane block has 256-byte slack per image)
     uint8_t *lldec = ws + dwt_plane_off(pl, L, n_images);
-    st = launch_aes_ctr(d_private, private_stride, lldec, pl.priv_b, pl.priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
+    const size_t lldec_stride = round_up(pl.priv_b, 16);
+    st = launch_aes_ctr(d_private, private_stride, lldec, lldec_stride, pl.priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
     if (st != FEDS_OK) return st;
 
     for (int l = L; l >= 1; --l) {
@@ -419,7 +423,7 @@ feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride,
         p.cw = w >> (l - 1); p.ch = h >> (l - 1);
         const int bw = w >> l, bh = h >> l;
         p.ll_band = reinterpret_cast<int16_t *>(ws + dwt_plane_off(pl, l, n_images));
-        p.ll_band_image_stride = (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
+        p.ll_band_image_stride = (l == L) ? lldec_stride / 2 : (size_t)c * bw * bh; p.ll_band_chan_stride = (size_t)bw * bh;
         p.pub = reinterpret_cast<int16_t *>(const_cast<uint8_t *>(d_public));
         p.pub_image_stride = public_stride / 2;
         p.pub_chan_stride = pl.pub_b / 2 / c;

@@ -52,6 +52,7 @@ struct DctParams {
     unsigned ws_n_sg;   // strip groups: ceil(n_images * nbr * nlr / 32)
     int ws_ahead;       // slabs a worker may run in front of its slowest hash warp
     uint32_t c128;      // = 128, opaque to the compiler (ws_lookup)
+    int generic_tiles;  // 1: digest-free path on the generic tile kernels even where the bulk-copy kernels apply (FEDS_FLAG_GENERIC_TILES)
 };
 
 // Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:

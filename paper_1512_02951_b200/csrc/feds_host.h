@@ -43,6 +43,10 @@ feds_status launch_fragment_fused(const DctParams &p, int c, cudaStream_t stream
 bool dct_ws_supported(const DctParams &p, int c);
 feds_status launch_fragment_ws(const DctParams &p, int c, cudaStream_t stream);
 feds_status launch_defragment_ws(const DctParams &p, int c, cudaStream_t stream);
+// ---- feds_k_dct_tma.cu: the digest-free tile kernels on bulk asynchronous copies (w % 32 == 0 and at least one tile per block row)
+bool dct_tma_supported(const DctParams &p, int c);
+feds_status launch_fragment_tma(const DctParams &p, int c, cudaStream_t stream);
+feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream, bool record_start);
 // ---- feds_k_dct_tile.cu: digest-free tile kernels and the registers-only leaf-hash kernel
 feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream);
 feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t stream, bool record_start);

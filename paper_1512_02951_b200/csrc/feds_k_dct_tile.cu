@@ -33,12 +33,14 @@ template <int C, int V> feds_status defrag(const DctParams &p, cudaStream_t s, b
 }  // namespace
 
 feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream) {
+    if (!p.generic_tiles && dct_tma_supported(p, c)) return launch_fragment_tma(p, c, stream);
     const int V = dct_vec_width(p.k);
 #define FEDS_V(CC) (V == 4 ? frag<CC, 4>(p, stream) : V == 2 ? frag<CC, 2>(p, stream) : frag<CC, 1>(p, stream))
     return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
 #undef FEDS_V
 }
 feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t stream, bool record_start) {
+    if (!p.generic_tiles && dct_tma_supported(p, c)) return launch_defragment_tma(p, c, stream, record_start);
     const int V = dct_vec_width(p.k);
 #define FEDS_V(CC) (V == 4 ? defrag<CC, 4>(p, stream, record_start) : V == 2 ? defrag<CC, 2>(p, stream, record_start) : defrag<CC, 1>(p, stream, record_start))
     return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);

@@ -358,6 +358,44 @@ def test_digest_free_tile_kernels(orc, b, n, w, h, c, k):
     assert torch.equal(out, d_imgs) and int(full.flags_out.abs().sum().item()) == 0
 
 
+# The digest-free path has two sets of tile kernels: the bulk-copy (TMA) ones (feds_dct_tma.cuh: w % 32 == 0, tiles of 32 / 64 blocks
+# in linear block order that may wrap into the next block row) and the generic ones (any w; FEDS_FLAG_GENERIC_TILES forces them).
+# Same arithmetic, other data movement: identical bytes both ways, the oracle's for these coefficient bytes, exact round trips
+# of either kernel's fragments through either inverse kernel.
+TMA_CASES = [(1, 512, 8, 1, 3), (1, 512, 512, 1, 2), (2, 576, 40, 1, 0), (1, 256, 8, 3, 3), (2, 288, 24, 3, 3), (3, 1920, 16, 3, 3),
+             (1, 1920, 1080, 3, 3), (2, 288, 40, 3, 4), (1, 320, 24, 3, 5), (1, 288, 24, 3, 62), (1, 256, 16, 3, 63), (2, 352, 24, 4, 7),
+             (1, 256, 8, 4, 0), (1, 800, 56, 4, 2), (1, 2048, 8, 3, 31), (5, 640, 72, 1, 9)]
+
+
+@pytest.mark.parametrize("n,w,h,c,k", TMA_CASES)
+def test_bulk_copy_and_generic_tile_kernels_agree(orc, b, n, w, h, c, k):
+    key, nonce = synth.key_nonce(w + 2 * k + c)
+    nonces = synth.batch_nonces(nonce, n)
+    imgs = np.stack([synth.image(w, h, c, seed=13 * w + i + k, rectangles=1) for i in range(n)])
+    d_imgs = torch.from_numpy(imgs).cuda()
+    d_nonces = torch.from_numpy(nonces).cuda()
+    tma, gen = b.DctBatch(n, w, h, c, k), b.DctBatch(n, w, h, c, k)
+    for t in (tma.priv, tma.pub, gen.priv, gen.pub):
+        t.fill_(0x3C)
+    tma.fragment(d_imgs, key, d_nonces, flags=b.FLAG_NO_DIGEST)
+    gen.fragment(d_imgs, key, d_nonces, flags=b.FLAG_NO_DIGEST | b.FLAG_GENERIC_TILES)
+    torch.cuda.synchronize()
+    assert torch.equal(tma.priv, gen.priv), "private fragments differ"
+    assert torch.equal(tma.pub, gen.pub), "public fragments differ"
+    for i in sorted({0, n - 1}):
+        pv = tma.priv[i * tma.priv_bytes:(i + 1) * tma.priv_bytes].cpu().numpy()
+        pb = tma.pub[i * tma.pub_bytes:(i + 1) * tma.pub_bytes].cpu().numpy()
+        coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[i].tobytes())
+        if w * h <= 1 << 19:
+            assert np.abs(coef - orc.dct_coefficients(imgs[i])).max() <= TOL
+        p2, q2, _ = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[i].tobytes())
+        assert (p2 == pv).all() and (q2 == pb).all()
+    for flags in (b.FLAG_NO_DIGEST, b.FLAG_NO_DIGEST | b.FLAG_GENERIC_TILES):
+        out = torch.full_like(d_imgs, 0x77)
+        tma.defragment(out, key, d_nonces, flags=flags)
+        assert torch.equal(out, d_imgs)
+
+
 # Steps 1-5 (and 6-8 with verification) run either in the warp-specialised fused kernels (feds_dct_ws.cuh: whole 8-block leaves,
 # k + 1 even) or as tile kernel + leaf-hash kernel (everything else); the library picks by shape and size, FEDS_FLAG_FORCE_FUSED /
 # FEDS_FLAG_FORCE_SPLIT override it. Both routes must produce the same bytes, digests, images and flags at any size.
