@@ -47,8 +47,8 @@ typedef enum {
                                   P:488-494), HBM-bound. d_digests is not written; defragment does not verify. */
 /* Route overrides (tests and profiling; results are byte-identical on every route). Without them the library picks the
  * route from the shape alone. A forced route that does not support the shape returns FEDS_ERR_BAD_PARAM. */
-#define FEDS_FLAG_FORCE_FUSED 2u /* DCT with digests: the warp-specialised fused kernel (needs (w/8) % 8 == 0 and k + 1 even) */
-#define FEDS_FLAG_FORCE_SPLIT 4u /* DCT with digests: digest-free tile kernel + leaf-hash kernel */
+#define FEDS_FLAG_FORCE_FUSED 2u /* DCT with digests: the warp-specialised fused kernel (needs w % 64 == 0 and w >= 256, gray: w >= 512) */
+#define FEDS_FLAG_FORCE_SPLIT 4u /* DCT with digests: digest-free tile kernel + leaf-hash kernel (what the library picks by itself) */
 #define FEDS_FLAG_DWT_TILED 8u   /* DWT: the tiled shared-memory level kernels instead of the register-streaming ones */
 #define FEDS_FLAG_GENERIC_TILES 16u /* DCT: the generic tile kernels (any w) even where the bulk-copy (TMA) tile kernels apply (w % 32 == 0) */
 
@@ -224,8 +224,8 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
 /*
  * Profiling hook (not part of the data path; thread-local): while set, every fragment/defragment call made on this
  * thread records ev_start immediately before and ev_stop immediately after its dominant kernel(s), on the call's stream:
- * DCT fragment: the fused kernel; DCT verified defragment: the leaf-hash kernel and the reconstruction kernel together;
- * digest-free DCT calls: the tile kernel; feds_verify_dct: the leaf-hash kernel; DWT path: the leaf-hashing kernel.
+ * DCT calls with digests (fragment, verified defragment, feds_verify_dct): the leaf-hash kernel, or the fused kernel on the
+ * FEDS_FLAG_FORCE_FUSED route; digest-free DCT calls: the tile kernel; DWT path: the leaf-hashing kernel.
  * Both are cudaEvent_t handles owned by the caller. Pass NULL, NULL to clear.
  */
 void feds_profile_events(void *ev_start, void *ev_stop);

@@ -7,6 +7,8 @@
  *   feds_debug_dct8x8_host   : forward (inverse=0) / inverse (inverse=1) 8x8 float32 transform, row-major; bit-identical to
  *                              what the kernels compute (every operation is an explicitly rounded IEEE-754 mul/add/fma).
  *   feds_debug_zigzag_host   : the kernels' zigzag table, out[z] = 8*row + col.
+ *   feds_debug_launch_count  : number of kernels this library has launched from the calling thread so far (a diagnostic counter,
+ *                              per thread like feds_last_cuda_error; bench.py reports its increase over the timed region).
  */
 #ifndef FEDS_DEBUG_H
 #define FEDS_DEBUG_H
@@ -22,6 +24,7 @@ void feds_debug_sha256_host(const uint8_t *msg, size_t n, uint8_t out[32]);
 void feds_debug_aes128_host(const uint8_t key[16], const uint8_t in[16], uint8_t out[16]);
 void feds_debug_dct8x8_host(const float in[64], float out[64], int inverse);
 void feds_debug_zigzag_host(int out[64]);
+unsigned long long feds_debug_launch_count(void);
 
 #ifdef __cplusplus
 }

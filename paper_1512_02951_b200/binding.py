@@ -31,7 +31,7 @@ SYMBOLS = [
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
     "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
-    "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host",
+    "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host", "feds_debug_launch_count",
 ]
 
 
@@ -82,6 +82,8 @@ def _load():
     lib.feds_debug_aes128_host.argtypes = [u8p, u8p, vp]
     lib.feds_debug_dct8x8_host.argtypes = [vp, vp, i]
     lib.feds_debug_zigzag_host.argtypes = [vp]
+    lib.feds_debug_launch_count.restype = C.c_ulonglong
+    lib.feds_debug_launch_count.argtypes = []
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
                  "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
                  "feds_fragment_dct_host", "feds_defragment_dct_host",
@@ -122,6 +124,11 @@ def _on_stream(stream, *tensors):
         for t in tensors:
             if t is not None and t.is_cuda:
                 t.record_stream(stream)
+
+
+def launch_count():
+    """kernels launched by the library from this thread so far (feds_debug_launch_count)"""
+    return int(lib.feds_debug_launch_count())
 
 
 def merkle_params():

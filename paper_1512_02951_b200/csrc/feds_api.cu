@@ -19,6 +19,7 @@ using namespace feds;
 namespace {
 thread_local int t_last_cuda_error = 0;
 thread_local cudaEvent_t t_prof_start = nullptr, t_prof_stop = nullptr;
+thread_local unsigned long long t_launches = 0;
 }  // namespace
 
 namespace feds {
@@ -34,6 +35,7 @@ int sm_count() {
 }
 cudaEvent_t prof_start_event() { return t_prof_start; }
 cudaEvent_t prof_stop_event() { return t_prof_stop; }
+void count_launch() { ++t_launches; }
 }  // namespace feds
 
 namespace {
@@ -99,32 +101,22 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.nbr = h / 8; p.nbc = w / 8; p.nlr = (p.nbc + G_BLOCKS - 1) / G_BLOCKS;
     p.leaves_per_image = (unsigned)c * p.nbr * p.nlr;
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
-    p.slot_stride = dct_slot_words(k);
     p.one = 1u;
-    p.n_groups = (unsigned)((p.total_leaves + 31) / 32);
-    p.ws_n_sg = (unsigned)(((unsigned long long)n_images * p.nbr * p.nlr + 31) / 32);
-    {   // the hash warps fetch 16 words at a time: the worker must be allowed far enough ahead to cover one fetch (feds_dct_ws.cuh)
-        const int wq = (63 - k) > 0 ? (63 - k) : (k + 1);
-        p.ws_ahead = std::max(2, (16 + wq - 1) / wq + 1);
-    }
-    p.c128 = 128u;
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
     aes128_expand_key_host(key, p.rk, h_aes);
 }
 
-// Which route fragments with digests. The warp-specialised fused kernel (feds_dct_ws.cuh) needs whole 8-block leaves and
-// 8/16-byte runs, and pays once its persistent grid is full; everything else runs as the digest-free tile kernel followed
-// by the leaf-hash kernel over what it wrote.
+// Which route runs the path with digests: the warp-specialised fused kernels (feds_dct_fused.cuh: w % 32 == 0, whole 8-block
+// leaves in linear block order) or the digest-free tile kernel and the leaf-hash kernel one after the other.
 constexpr unsigned DCT_FLAGS = FEDS_FLAG_NO_DIGEST | FEDS_FLAG_FORCE_FUSED | FEDS_FLAG_FORCE_SPLIT | FEDS_FLAG_GENERIC_TILES;
 enum class Route { Fused, Split, Unsupported };
 Route pick_route(const DctParams &p, int c, unsigned flags) {
-    const bool ws_ok = dct_ws_supported(p, c);
+    const bool ws_ok = dct_fused_supported(p, c);
     if (flags & FEDS_FLAG_FORCE_FUSED) return ws_ok ? Route::Fused : Route::Unsupported;
     if (flags & FEDS_FLAG_FORCE_SPLIT) return Route::Split;
-    if (ws_ok && p.n_groups >= 16u * (unsigned)sm_count()) return Route::Fused;
-    return Route::Split;
+    return Route::Split;   // measured faster at every size since the tile kernels moved to bulk copies
 }
 
 feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
@@ -158,12 +150,11 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
         const Route route = pick_route(p, c, flags);
         if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;
         if (route == Route::Fused) {
-            st = launch_fragment_ws(p, c, stream);
+            st = launch_fragment_fused(p, c, stream);
         } else {
-            st = launch_fragment_tile(p, c, stream);   // records the profiling start; the stop follows the leaf hash
+            st = launch_fragment_tile(p, c, stream, false);
             if (st != FEDS_OK) return st;
-            st = launch_leaves_hash(p, c, stream);
-            if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
+            st = launch_leaves_hash(p, c, stream, true);   // the dominant kernel: the profiling events bracket it
         }
         if (st != FEDS_OK) return st;
         if (pl.nl > 1) {
@@ -175,7 +166,7 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
             if (st != FEDS_OK) return st;
         }
     } else {
-        st = launch_fragment_tile(p, c, stream);
+        st = launch_fragment_tile(p, c, stream, true);
         if (st != FEDS_OK) return st;
     }
     return FEDS_OK;
@@ -233,10 +224,9 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
         const Route route = pick_route(p, c, flags);
         if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;
         if (route == Route::Fused) {
-            st = launch_defragment_ws(p, c, stream);
+            st = launch_defragment_fused(p, c, stream);
         } else {
-            if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-            st = launch_leaves_hash(p, c, stream);
+            st = launch_leaves_hash(p, c, stream, true);
             if (st != FEDS_OK) return st;
             st = launch_defragment_tile(p, c, stream, false);
         }
@@ -266,9 +256,7 @@ feds_status verify_dct_impl(const uint8_t *d_private, size_t private_stride, con
     p.priv = const_cast<uint8_t *>(d_private); p.priv_stride = private_stride;
     p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
     p.leaves = verification_leaves(pl, n_images, static_cast<uint8_t *>(d_workspace));
-    if (t_prof_start) FEDS_CUDA(cudaEventRecord(t_prof_start, stream));
-    st = launch_leaves_hash(p, c, stream);
-    if (t_prof_stop) FEDS_CUDA(cudaEventRecord(t_prof_stop, stream));
+    st = launch_leaves_hash(p, c, stream, true);
     if (st != FEDS_OK) return st;
     return finish_verification(p, pl, n_images, k, static_cast<uint8_t *>(d_workspace), d_expected, d_flags, stream);
 }
@@ -737,6 +725,8 @@ void feds_profile_events(void *ev_start, void *ev_stop) {
 }
 
 // ------------------------------------------------------------------------------------------------ host self-checks
+unsigned long long feds_debug_launch_count(void) { return t_launches; }
+
 void feds_debug_sha256_host(const uint8_t *msg, size_t n, uint8_t out[32]) {
     uint32_t H[8], w[16];
     sha256_init(H);

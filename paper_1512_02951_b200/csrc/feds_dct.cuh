@@ -1,21 +1,7 @@
-// feds_dct.cuh — the fused fragment kernel of the DCT path and the block load / store /
-// slot helpers the other DCT kernels share (feds_dct_tile.cuh: digest-free kernels, leaf-hash kernel), sm_100a.
-//
-// One thread owns one Merkle leaf = up to G consecutive 8x8 blocks of one block row of one channel
-// (DESIGN.md 2.1). For each block it: loads the 8x8 pixels, runs the separable FP32 DCT in 64 registers,
-// splits the coefficients in zigzag order into its private / public words, AES-128-CTR-encrypts the private
-// words (shared-memory T-tables, sequential keystream along the leaf), writes both runs to HBM, and absorbs the
-// stored bytes of both fragments into two running SHA-256 states fed from a per-lane shared-memory slot (one
-// inlined compression site). Pixels are read once; coefficients are written once; only 2 x 32 B of leaf digest
-// per leaf go to the workspace.
-//
-// Template parameter V = words per vector access of a coefficient run, the largest of {4, 2, 1} dividing
-// P = k+1 (then it divides Q = 64-P too, and every run starts 4V-byte aligned):
-//   V = 4 / 2 : each lane moves its own runs with 128 / 64-bit accesses straight from / to registers; no warp
-//               cooperation, no barrier in the block loop.
-//   k + 1 odd : 4-byte runs would scatter 64 stores per block over 32 lines each; the host routes those k to the tile
-//               kernel followed by the leaf-hash kernel (feds_dct_tile.cuh), which measured 2-4 % faster than a
-//               warp-cooperative copy inside this kernel did.
+// feds_dct.cuh — what the DCT-path kernels share (sm_100a): the parameter block, vector run access, pixel <-> float32 block load /
+// store for the generic tile kernels, leaf geometry, per-image nonces, digest store. The kernels themselves live in
+// feds_dct_tile.cuh (generic tile kernels, leaf-hash kernel), feds_dct_tma.cuh (bulk-copy tile kernels) and feds_dct_fused.cuh
+// (warp-specialised fused kernels with digests).
 #pragma once
 #include "feds_device.cuh"
 
@@ -23,11 +9,7 @@ namespace feds {
 
 static __device__ const AesTables g_aes = make_aes_tables();   // one copy per translation unit
 
-constexpr int DCT_THREADS = 512;     // one persistent CTA per SM: 16 warps, 4 per scheduler (8 warps when the slots of 16 do not fit)
-constexpr int DCT_CTAS_PER_SM = 1;
-constexpr size_t DCT_SMEM_MAX = 227 * 1024;
 constexpr int AES_TABLE_WORDS = 1024;
-constexpr int CA = 16;  // carry area: a SHA-256 block is 16 words, at most 15 (16 - V) words wait between blocks
 
 struct DctParams {
     const uint8_t *images;  // fragment: input images; defragment: unused
@@ -45,30 +27,13 @@ struct DctParams {
     int nbr, nbc, nlr;
     unsigned leaves_per_image;  // C * nbr * nlr
     unsigned long long total_leaves;
-    int slot_stride;  // words per lane slot
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
-    unsigned n_groups;  // ceil(total_leaves / 32): one group = the 32 leaves one warp owns at a time
-    // warp-specialised kernels (feds_dct_ws.cuh)
-    unsigned ws_n_sg;   // strip groups: ceil(n_images * nbr * nlr / 32)
-    int ws_ahead;       // slabs a worker may run in front of its slowest hash warp
-    uint32_t c128;      // = 128, opaque to the compiler (ws_lookup)
     int generic_tiles;  // 1: digest-free path on the generic tile kernels even where the bulk-copy kernels apply (FEDS_FLAG_GENERIC_TILES)
 };
 
-// Slot layout (word offsets in a lane's slot), P private and Q = 64 - P public words per block:
-//   [0, 16)        private carry        [16, 16+P)       private words of the current block, index z
-//   [16+P, 32+P)   public carry         [32+P, 96)       public words of the current block, index z (address 32 + z)
-// plus slack so that the <= 32 padding words of the final phase fit behind the public carry area.
-// The stride makes per-lane V-word accesses conflict-free: odd (V=1), 2 mod 4 (V=2), 4 mod 8 (V=4).
+// words per vector access of a coefficient run: the largest of {4, 2, 1} dividing P = k + 1 (then it divides Q = 64 - P too, and
+// every run starts 4V-byte aligned)
 __host__ __device__ inline int dct_vec_width(int k) { return ((k + 1) % 4 == 0) ? 4 : ((k + 1) % 2 == 0) ? 2 : 1; }
-__host__ __device__ inline int dct_slot_words(int k) {
-    const int Q = 63 - k, V = dct_vec_width(k);
-    int wds = 2 * CA + 64 + (Q < 32 ? 32 - Q : 0) + 8;  // + 8: the waiting stream's chaining value (dct_stash_offset)
-    while (wds % (2 * V) != V) ++wds;
-    return wds;
-}
-
-__host__ __device__ inline int dct_stash_offset(int k) { const int Q = 63 - k; return 2 * CA + 64 + (Q < 32 ? 32 - Q : 0); }
 
 template <int V> struct VecT;
 template <> struct VecT<1> { using type = uint32_t; };
@@ -253,106 +218,6 @@ __device__ __forceinline__ void load_nonce(const DctParams &p, int n, uint32_t (
     }
 }
 
-// One SHA-256 stream living in a lane's slot: `carry` words wait at [base+16-carry, base+16), `fresh` new words
-// were just written at [base+16, base+16+fresh). Compress every full 16-word block, slide the rest down.
-struct ShaMeta {
-    int base;
-    int carry;
-    int fresh;
-    unsigned total_words;
-};
-struct ShaStream {
-    uint32_t H[8];
-    int base;
-    int carry;
-    int fresh;
-    unsigned total_words;  // message length of the whole leaf in 32-bit words (0: stream unused)
-};
-
-// Only the stream being absorbed keeps its chaining value in registers; the other one's waits in the lane's slot at
-// word offset `hoff` (8 words). 16 fewer live registers across the compression loop than a register swap.
-template <int V>
-__device__ __forceinline__ void swap_streams(uint32_t *my, int hoff, ShaStream &a, ShaMeta &b) {
-#pragma unroll
-    for (int i = 0; i < 8; i += V) {
-        uint32_t t[V], u[V];
-        vec_load<V>(my + hoff + i, t);
-#pragma unroll
-        for (int j = 0; j < V; ++j) u[j] = a.H[i + j];
-        vec_store<V>(my + hoff + i, u);
-#pragma unroll
-        for (int j = 0; j < V; ++j) a.H[i + j] = t[j];
-    }
-    int t;
-    t = a.base; a.base = b.base; b.base = t;
-    t = a.carry; a.carry = b.carry; b.carry = t;
-    t = a.fresh; a.fresh = b.fresh; b.fresh = t;
-    const unsigned u = a.total_words; a.total_words = b.total_words; b.total_words = u;
-}
-template <int V>
-__device__ __forceinline__ void stash_init(uint32_t *my, int hoff) {
-    uint32_t H[8];
-    sha256_init(H);
-#pragma unroll
-    for (int i = 0; i < 8; i += V) {
-        uint32_t u[V];
-#pragma unroll
-        for (int j = 0; j < V; ++j) u[j] = H[i + j];
-        vec_store<V>(my + hoff + i, u);
-    }
-}
-template <int V>
-__device__ __forceinline__ void stash_read(const uint32_t *my, int hoff, uint32_t (&H)[8]) {
-#pragma unroll
-    for (int i = 0; i < 8; i += V) {
-        uint32_t t[V];
-        vec_load<V>(my + hoff + i, t);
-#pragma unroll
-        for (int j = 0; j < V; ++j) H[i + j] = t[j];
-    }
-}
-
-// Append the FIPS 180-4 5.1.1 padding for a message of `total_words` 32-bit words after the carried words.
-// Slot words are little-endian data words (byte-swapped when loaded into W), so the padding is written pre-swapped.
-__device__ __forceinline__ void write_padding(uint32_t *my, ShaStream &s) {
-    const int n = s.carry;
-    int tot = n + 3;                      // 0x80 word + 64-bit length
-    tot = (tot + 15) & ~15;               // 16 or 32
-    const int fresh = tot - n;
-    uint32_t *dst = my + s.base + CA;
-    dst[0] = 0x00000080u;
-    for (int i = 1; i < fresh - 2; ++i) dst[i] = 0u;
-    const unsigned long long bits = (unsigned long long)s.total_words * 32ull;
-    dst[fresh - 2] = bswap32((uint32_t)(bits >> 32));
-    dst[fresh - 1] = bswap32((uint32_t)bits);
-    s.fresh = fresh;
-}
-
-// `VA` = alignment (in words) every quantity of this stream is a multiple of: the window start, carry and fresh.
-template <int VA>
-__device__ __forceinline__ void absorb(uint32_t *my, ShaStream &s, const uint32_t one) {
-    int cnt = s.carry + s.fresh;
-    int ptr = s.base + CA - s.carry;
-    while (cnt >= 16) {
-        uint32_t w[16];
-#pragma unroll
-        for (int i = 0; i < 16; i += VA) {
-            uint32_t x[VA];
-            vec_load<VA>(my + ptr + i, x);
-#pragma unroll
-            for (int t = 0; t < VA; ++t) w[i + t] = bswap32(x[t]);
-        }
-        sha256_compress_rolled_fma(s.H, w, one);
-        ptr += 16;
-        cnt -= 16;
-    }
-    const int dst = s.base + CA - cnt;
-    if (dst != ptr)
-        for (int i = 0; i < cnt; ++i) my[dst + i] = my[ptr + i];  // dst <= ptr: ascending copy is safe
-    s.carry = cnt;
-    s.fresh = 0;
-}
-
 __device__ __forceinline__ void store_digest(uint8_t *dst, const uint32_t (&H)[8]) {
     uint4 a, b;
     a.x = bswap32(H[0]); a.y = bswap32(H[1]); a.z = bswap32(H[2]); a.w = bswap32(H[3]);
@@ -365,124 +230,6 @@ __device__ __forceinline__ void load_aes_tables(uint32_t *sT) {
     const uint32_t *src = &g_aes.T[0][0];
     for (int i = threadIdx.x; i < AES_TABLE_WORDS; i += blockDim.x) sT[i] = src[i];
     __syncthreads();
-}
-
-// Sequential CTR keystream along one private run: V words starting at word `wi` (absolute 32-bit word index in
-// the image's private stream, a multiple of V); a new AES block is computed only when a 16-byte boundary is crossed.
-struct Keystream {
-    uint32_t ks[4];
-    unsigned long long blk;
-};
-template <int V, typename Tab>
-__device__ __forceinline__ void keystream_words(Keystream &K, const Tab sT, const uint32_t *rk, const uint32_t (&nonce)[4],
-                                                unsigned long long wi, uint32_t (&out)[V]) {
-    const unsigned long long blk = wi >> 2;
-    if (V == 4 || blk != K.blk) {
-        ctr_block(nonce, blk, K.ks);
-        aes128_encrypt(sT, rk, K.ks);
-        K.blk = blk;
-    }
-    if (V == 4) {
-#pragma unroll
-        for (int t = 0; t < V; ++t) out[t] = K.ks[t];
-    } else if (V == 2) {
-        const bool up = (wi & 2) != 0;
-        out[0] = up ? K.ks[2] : K.ks[0];
-        out[1 % V] = up ? K.ks[3] : K.ks[1];
-    } else {
-        const int sel = (int)(wi & 3);
-        out[0] = sel == 0 ? K.ks[0] : sel == 1 ? K.ks[1] : sel == 2 ? K.ks[2] : K.ks[3];
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// fragment: steps 1-5. V = 2 or 4 (when k + 1 is odd the host takes the tile kernel + leaf-hash kernel route instead).
-// ------------------------------------------------------------------------------------------------------------
-template <int C, int V>
-__global__ void __launch_bounds__(DCT_THREADS, DCT_CTAS_PER_SM) fragment_dct_kernel(const __grid_constant__ DctParams p) {
-    extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *sT = smem;
-    load_aes_tables(sT);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *wslots = smem + AES_TABLE_WORDS + warp * 32 * p.slot_stride;
-    uint32_t *my = wslots + lane * p.slot_stride;
-    constexpr ZigzagTable ZZ = make_zigzag();
-
-    const int k = p.k, P = k + 1, Q = 63 - k;
-    uint32_t *mp = my + CA;      // private words of the current block, indexed by z
-    uint32_t *mq = my + 2 * CA;  // public words of the current block, indexed by z (z >= P)
-#pragma unroll 1
-    for (unsigned grp = (unsigned)warp * gridDim.x + blockIdx.x; grp < p.n_groups; grp += (blockDim.x >> 5) * gridDim.x) {
-    const LeafCoord L = decode_leaf<C>(p, (unsigned long long)grp * 32 + lane);
-    const uint8_t *img = p.images + (size_t)L.n * p.image_stride;
-    uint32_t *pub_dst = reinterpret_cast<uint32_t *>(p.pub + (size_t)L.n * p.pub_stride) + (size_t)L.b0 * Q;
-    uint32_t *priv_dst = reinterpret_cast<uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
-    uint32_t nonce[4];
-    load_nonce(p, L.n, nonce);
-
-    // cur = public stream, oth = private stream (swapped twice per phase). The public stream goes first so that in the
-    // final phase the private stream's padding may spill into the (then finished) public region.
-    ShaStream cur;
-    ShaMeta oth;
-    const int hoff = dct_stash_offset(k);
-    sha256_init(cur.H);
-    stash_init<V>(my, hoff);
-    cur.base = CA + P; cur.carry = 0; cur.fresh = 0; cur.total_words = (unsigned)(L.nblk * Q);
-    oth.base = 0; oth.carry = 0; oth.fresh = 0; oth.total_words = (unsigned)(L.nblk * P);
-    Keystream K;
-    K.blk = ~0ull;
-    const unsigned long long priv_word0 = (unsigned long long)L.b0 * P;
-
-#pragma unroll 1
-    for (int s = 0; s <= G_BLOCKS; ++s) {
-        if (s < G_BLOCKS) {
-            const bool act = s < L.nblk;
-            uint32_t *pq = pub_dst + (size_t)s * Q - P;  // public run of this block, indexed by z
-            uint32_t *pv = priv_dst + (size_t)s * P;      // private run of this block, indexed by z
-            if (act) {
-                float v[64];
-                load_block<C>(img, p.w, 8 * L.br, 8 * (L.g * G_BLOCKS + s), L.c, v);
-                dct8x8(v);
-#pragma unroll
-                for (int g = 0; g < 64; g += V) {
-                    uint32_t x[V];
-#pragma unroll
-                    for (int t = 0; t < V; ++t) x[t] = __float_as_uint(v[ZZ.pos[g + t]]);
-                    if (g < P) {
-                        vec_store<V>(mp + g, x);   // plaintext; encrypted in place below
-                    } else {
-                        vec_store<V>(mq + g, x);
-                        vec_store<V>(pq + g, x);
-                    }
-                }
-                const unsigned long long w0 = priv_word0 + (unsigned long long)s * P;
-#pragma unroll 1
-                for (int j = 0; j < P; j += V) {
-                    uint32_t ks[V], x[V];
-                    keystream_words<V>(K, sT, p.rk, nonce, w0 + j, ks);
-                    vec_load<V>(mp + j, x);
-#pragma unroll
-                    for (int t = 0; t < V; ++t) x[t] ^= ks[t];
-                    vec_store<V>(mp + j, x);
-                    vec_store<V>(pv + j, x);
-                }
-            }
-            cur.fresh = act ? Q : 0; oth.fresh = act ? P : 0;
-        }
-#pragma unroll 1
-        for (int it = 0; it < 2; ++it) {
-            if (s == G_BLOCKS && cur.total_words != 0u) write_padding(my, cur);
-            absorb<V>(my, cur, p.one);
-            swap_streams<V>(my, hoff, cur, oth);
-        }
-    }
-    if (L.valid) {
-        const size_t nl = p.leaves_per_image;
-        if (Q > 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * nl + L.li) * 32, cur.H);
-        stash_read<V>(my, hoff, cur.H);  // after an even number of swaps the private stream is the stashed one
-        store_digest(p.leaves + (((size_t)L.n * 2 + 0) * nl + L.li) * 32, cur.H);
-    }
-    }
 }
 
 }  // namespace feds

@@ -50,17 +50,27 @@ __device__ __forceinline__ uint32_t t0_lookup(const T0Lane &T, uint32_t word) {
     const uint32_t v = *reinterpret_cast<const uint32_t *>(T.tab + o);
     return TABLE == 0 ? v : __funnelshift_l(v, v, 8 * TABLE);
 }
-template <typename RkPtr>
+// ROLLED: the nine middle rounds as a loop (round keys indexed at run time): a tenth of the code, for kernels whose hot code
+// must share the SM's 32 KB instruction cache with a SHA-256 loop (feds_dct_fused.cuh).
+template <bool ROLLED = false, typename RkPtr>
 __device__ __forceinline__ void aes128_encrypt(const T0Lane &T, const RkPtr rk, uint32_t (&s)[4]) {
     uint32_t s0 = s[0] ^ rk[0], s1 = s[1] ^ rk[1], s2 = s[2] ^ rk[2], s3 = s[3] ^ rk[3];
-#pragma unroll
-    for (int r = 1; r < 10; ++r) {
-        const uint32_t t0 = t0_lookup<0, 0>(T, s0) ^ t0_lookup<1, 1>(T, s1) ^ t0_lookup<2, 2>(T, s2) ^ t0_lookup<3, 3>(T, s3) ^ rk[4 * r + 0];
-        const uint32_t t1 = t0_lookup<0, 0>(T, s1) ^ t0_lookup<1, 1>(T, s2) ^ t0_lookup<2, 2>(T, s3) ^ t0_lookup<3, 3>(T, s0) ^ rk[4 * r + 1];
-        const uint32_t t2 = t0_lookup<0, 0>(T, s2) ^ t0_lookup<1, 1>(T, s3) ^ t0_lookup<2, 2>(T, s0) ^ t0_lookup<3, 3>(T, s1) ^ rk[4 * r + 2];
-        const uint32_t t3 = t0_lookup<0, 0>(T, s3) ^ t0_lookup<1, 1>(T, s0) ^ t0_lookup<2, 2>(T, s1) ^ t0_lookup<3, 3>(T, s2) ^ rk[4 * r + 3];
-        s0 = t0; s1 = t1; s2 = t2; s3 = t3;
+#define FEDS_ROUND(r)                                                                                                                       \
+    {                                                                                                                                       \
+        const uint32_t t0 = t0_lookup<0, 0>(T, s0) ^ t0_lookup<1, 1>(T, s1) ^ t0_lookup<2, 2>(T, s2) ^ t0_lookup<3, 3>(T, s3) ^ rk[4 * (r) + 0]; \
+        const uint32_t t1 = t0_lookup<0, 0>(T, s1) ^ t0_lookup<1, 1>(T, s2) ^ t0_lookup<2, 2>(T, s3) ^ t0_lookup<3, 3>(T, s0) ^ rk[4 * (r) + 1]; \
+        const uint32_t t2 = t0_lookup<0, 0>(T, s2) ^ t0_lookup<1, 1>(T, s3) ^ t0_lookup<2, 2>(T, s0) ^ t0_lookup<3, 3>(T, s1) ^ rk[4 * (r) + 2]; \
+        const uint32_t t3 = t0_lookup<0, 0>(T, s3) ^ t0_lookup<1, 1>(T, s0) ^ t0_lookup<2, 2>(T, s1) ^ t0_lookup<3, 3>(T, s2) ^ rk[4 * (r) + 3]; \
+        s0 = t0; s1 = t1; s2 = t2; s3 = t3;                                                                                                 \
     }
+    if (ROLLED) {
+#pragma unroll 1
+        for (int r = 1; r < 10; ++r) FEDS_ROUND(r)
+    } else {
+#pragma unroll
+        for (int r = 1; r < 10; ++r) FEDS_ROUND(r)
+    }
+#undef FEDS_ROUND
     // final round: SubBytes + ShiftRows; T0 = (2S, S, S, 3S): S is byte 1 (and 2) of every T0 word
 #define FEDS_LAST(a, b, c, d)                                                                                          \
     __byte_perm(__byte_perm(t0_lookup<0, 0>(T, a), t0_lookup<1, 0>(T, b), 0x3251), __byte_perm(t0_lookup<2, 0>(T, c), t0_lookup<3, 0>(T, d), 0x5210), 0x7610)

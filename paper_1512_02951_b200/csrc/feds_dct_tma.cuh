@@ -145,22 +145,33 @@ __device__ __forceinline__ void tma_move_runs(const DctParams &p, const TmaTile 
 // ------------------------------------------------------------------------------------------------------------ pixels <-> registers
 // 32768 + x, exactly: the byte goes to mantissa bits 8..15 of 2^15
 __device__ __forceinline__ float byte_to_biased_float(uint32_t word, int pos) { return __uint_as_float(__byte_perm(word, 0x47000000u, 0x7404u + ((uint32_t)pos << 4))); }
+__device__ __forceinline__ uint2 lds64(uint32_t a) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+    return v;
+}
+// `blk` = shared-memory address of the block's first pixel row
 template <int C, int CH>
-__device__ __forceinline__ void load_block_biased(const uint8_t *blk, uint32_t pitch, float (&v)[64]) {
+__device__ __forceinline__ void load_block_biased(uint32_t blk, uint32_t pitch, float (&v)[64]) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
-        const uint8_t *row = blk + r * pitch;
+        const uint32_t row = blk + r * pitch;
         if (C == 1) {
-            const uint2 q = *reinterpret_cast<const uint2 *>(row);
+            const uint2 q = lds64(row);
 #pragma unroll
             for (int i = 0; i < 4; ++i) { v[8 * r + i] = byte_to_biased_float(q.x, i); v[8 * r + 4 + i] = byte_to_biased_float(q.y, i); }
         } else if (C == 3) {
-            const uint2 q0 = reinterpret_cast<const uint2 *>(row)[0], q1 = reinterpret_cast<const uint2 *>(row)[1], q2 = reinterpret_cast<const uint2 *>(row)[2];
+            const uint2 q0 = lds64(row), q1 = lds64(row + 8), q2 = lds64(row + 16);
             const uint32_t wd[6] = {q0.x, q0.y, q1.x, q1.y, q2.x, q2.y};
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[8 * r + i] = byte_to_biased_float(wd[(3 * i + CH) >> 2], (3 * i + CH) & 3);
         } else {
-            const uint4 a = reinterpret_cast<const uint4 *>(row)[0], b = reinterpret_cast<const uint4 *>(row)[1];
+            const uint4 a = lds128(row), b = lds128(row + 16);
             const uint32_t wd[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[8 * r + i] = byte_to_biased_float(wd[i], CH);
@@ -192,7 +203,7 @@ template <int C>
 __device__ __forceinline__ void tma_block_dct(const uint8_t *s_pix, const TmaTile &T, int j, int ch, float (&v)[64]) {
     uint32_t off, pitch;
     tma_pixel_slot<C>(T, j, off, pitch);
-    const uint8_t *blk = s_pix + off;
+    const uint32_t blk = smem_u32(s_pix) + off;
     if (C == 1) load_block_biased<1, 0>(blk, pitch, v);
     else if (ch == 0) load_block_biased<C, 0>(blk, pitch, v);   // warp-uniform branches: the channel selects immediates
     else if (ch == 1) load_block_biased<C, 1>(blk, pitch, v);
@@ -203,7 +214,7 @@ __device__ __forceinline__ void tma_block_dct(const uint8_t *s_pix, const TmaTil
 
 // AES-128-CTR over the staged private runs of a tile by the whole group (k + 1 not a multiple of 4): every counter block that
 // overlaps a run is computed once. Run c holds words [W0_c, W0_c + nb * P) of the image's private stream.
-template <int C>
+template <int C, bool SMALL = false>
 __device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lane &sT, const TmaTile &T, uint32_t *s_priv, int RSP, int P, int tid) {
     constexpr int THREADS = TmaShape<C>::THREADS, TB = TmaShape<C>::TB;
     uint32_t nonce[4];
@@ -219,7 +230,7 @@ __device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lan
         if (first >= nw) continue;
         uint32_t ks[4];
         ctr_block(nonce, blk, ks);
-        aes128_encrypt(sT, p.rk, ks);
+        aes128_encrypt<SMALL>(sT, p.rk, ks);
         uint32_t *run = s_priv + c * RSP;
         if (first >= 0 && first + 4 <= nw && (first & 3) == 0) {
             uint4 x = *reinterpret_cast<uint4 *>(run + first);
@@ -235,6 +246,7 @@ __device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lan
     }
 }
 // AES-128-CTR of one block's own private words in the stage (4 | k + 1: they are whole counter blocks)
+template <bool SMALL = false>
 __device__ __forceinline__ void tma_aes_ctr_own(const DctParams &p, const T0Lane &sT, int n, unsigned long long w0, int P, uint32_t *my_priv) {
     uint32_t nonce[4];
     load_nonce(p, n, nonce);
@@ -242,7 +254,7 @@ __device__ __forceinline__ void tma_aes_ctr_own(const DctParams &p, const T0Lane
     for (int g = 0; g < P; g += 4) {
         uint32_t ks[4];
         ctr_block(nonce, (w0 + g) >> 2, ks);
-        aes128_encrypt(sT, p.rk, ks);
+        aes128_encrypt<SMALL>(sT, p.rk, ks);
         uint4 x = *reinterpret_cast<uint4 *>(my_priv + g);
         x.x ^= ks[0]; x.y ^= ks[1]; x.z ^= ks[2]; x.w ^= ks[3];
         *reinterpret_cast<uint4 *>(my_priv + g) = x;
@@ -278,7 +290,7 @@ __device__ __forceinline__ TmaGroup<C> tma_group_setup(uint32_t *smem, int k, in
 // One tile, from the pixel tile in shared memory (already waited for) to the stage: DCT, zigzag split, AES. Ends with the
 // barrier after which the elected thread may issue the bulk stores. `pre_stage` runs between the arithmetic and the first write
 // to the stage (the caller waits there until the previous tile's stores have read the stage).
-template <int C, int V, typename PreStage>
+template <int C, int V, bool SMALL = false, typename PreStage>
 __device__ __forceinline__ void tma_fragment_tile(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, const uint8_t *s_pix,
                                                   PreStage &&pre_stage) {
     constexpr ZigzagTable ZZ = make_zigzag();
@@ -298,11 +310,11 @@ __device__ __forceinline__ void tma_fragment_tile(const DctParams &p, const T0La
             for (int q = 0; q < V; ++q) x[q] = __float_as_uint(v[ZZ.pos[g + q]]);
             vec_store<V>(g < P ? my_priv + g : my_pub + g, x);
         }
-        if (V == 4) tma_aes_ctr_own(p, sT, T.n, ((unsigned long long)G.ch * p.nbr * p.nbc + T.B0 + G.j) * P, P, my_priv);
+        if (V == 4) tma_aes_ctr_own<SMALL>(p, sT, T.n, ((unsigned long long)G.ch * p.nbr * p.nbc + T.B0 + G.j) * P, P, my_priv);
     }
     if (V != 4) {
         group_sync(G.gid, THREADS);
-        tma_aes_ctr_runs<C>(p, sT, T, G.s_priv, G.RSP, P, G.tid);
+        tma_aes_ctr_runs<C, SMALL>(p, sT, T, G.s_priv, G.RSP, P, G.tid);
     }
     fence_proxy_async();
     group_sync(G.gid, THREADS);
@@ -341,13 +353,13 @@ __global__ void __launch_bounds__(TmaShape<C>::CTA, 1) fragment_dct_tma_kernel(c
 
 // ------------------------------------------------------------------------------------------------------------ defragment: steps 6-8
 // stage (already waited for) -> decrypt, merge, IDCT -> packed rows of this thread's block in registers (2 words per row)
-template <int C, int V>
+template <int C, int V, bool SMALL = false>
 __device__ __forceinline__ void tma_defragment_block(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, uint32_t (&rows)[16]) {
     constexpr ZigzagTable ZZ = make_zigzag();
     const int P = p.k + 1, Q = 63 - p.k;
     uint32_t *my_pub = G.s_pub + G.ch * G.RSQ + G.j * Q - P;   // indexed by z
     uint32_t *my_priv = G.s_priv + G.ch * G.RSP + G.j * P;
-    if (V == 4) tma_aes_ctr_own(p, sT, T.n, ((unsigned long long)G.ch * p.nbr * p.nbc + T.B0 + G.j) * P, P, my_priv);
+    if (V == 4) tma_aes_ctr_own<SMALL>(p, sT, T.n, ((unsigned long long)G.ch * p.nbr * p.nbc + T.B0 + G.j) * P, P, my_priv);
     float v[64];
 #pragma unroll
     for (int g = 0; g < 64; g += V) {
@@ -399,16 +411,16 @@ __device__ __forceinline__ void tma_interleave(const TmaTile &T, const uint8_t *
 // One tile from the stage (already waited for) to the out tile in shared memory, ending with the barrier after which the elected
 // thread may issue the pixel stores. `stage_read` runs right after the barrier that follows the last read of the stage (the caller
 // refills the stage there); before that barrier the elected thread has waited for the previous out tile to be read.
-template <int C, int V, typename StageRead>
+template <int C, int V, bool SMALL = false, typename StageRead>
 __device__ __forceinline__ void tma_defragment_tile(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, StageRead &&stage_read) {
     constexpr int THREADS = TmaShape<C>::THREADS, TB = TmaShape<C>::TB;
     const bool act = G.j < T.nb;
     if (V != 4) {
-        tma_aes_ctr_runs<C>(p, sT, T, G.s_priv, G.RSP, p.k + 1, G.tid);
+        tma_aes_ctr_runs<C, SMALL>(p, sT, T, G.s_priv, G.RSP, p.k + 1, G.tid);
         group_sync(G.gid, THREADS);
     }
     uint32_t rows[16];
-    if (act) tma_defragment_block<C, V>(p, sT, G, T, rows);
+    if (act) tma_defragment_block<C, V, SMALL>(p, sT, G, T, rows);
     if (G.tid == 0) bulk_wait_read0();   // the previous tile's pixel stores have read the out tile
     group_sync(G.gid, THREADS);
     stage_read();

@@ -205,6 +205,7 @@ struct CtrParams {
     const uint8_t *d_nonces;          // device uint8[n_msgs][16], or nullptr: nonce_be for the single message
     uint32_t nonce_be[4];
     uint32_t rk[44];
+    uint32_t c128;                    // = 128, opaque to the compiler (rep_lookup)
 };
 __device__ __forceinline__ void ctr_load_nonce(const CtrParams &p, unsigned m, uint32_t (&nonce)[4]) {
     if (p.d_nonces) {
@@ -222,36 +223,38 @@ struct ReplTable {
     __device__ __forceinline__ uint32_t operator[](unsigned i) const { return b[i * REPL]; }
 };
 
-// The ten rounds on the 32-fold replicated four-table layout, addressed in bytes so that every lookup costs two ALU-pipe
-// instructions (shift; mask-and-or-in-the-lane) and no address arithmetic: entry x of table t, copy l sits at byte
-// t * 32768 + x * 128 + l * 4. `lane4` = 4 * lane. Same arithmetic as aes128_encrypt (FIPS-197 5.1, T-table form).
-__device__ __forceinline__ uint32_t rep_lookup(const char *tab, uint32_t word, int byte, int table, uint32_t lane4) {
-    uint32_t o;   // (right shifts as multiply-high on the FMA pipe were tried here: IMAD.HI is half rate, 9 % slower)
-    if (byte == 0) o = ((word << 7) & 0x7f80u) | lane4;
-    else if (byte == 1) o = ((word >> 1) & 0x7f80u) | lane4;
-    else if (byte == 2) o = ((word >> 9) & 0x7f80u) | lane4;
-    else o = ((word >> 17) & 0x7f80u) | lane4;
-    return *reinterpret_cast<const uint32_t *>(tab + table * 32768 + o);
+// The ten rounds on the 32-fold replicated four-table layout (entry x of table t, copy l at byte t * 32768 + x * 128 + l * 4;
+// lane l reads copy l, which lies in bank l: every lookup is one wavefront). A lookup costs ONE ALU-pipe instruction (PRMT: the
+// byte, zero-extended), one IMAD on the FMA pipe (byte * 128 + lane base; the multiplier is a run-time 128 so that ptxas keeps it a
+// multiply-add instead of a shift and an add on the ALU pipe) and the LDS, whose immediate offset selects the table: 24 ALU-pipe
+// instructions per round against 40 for shift + mask-or-lane. Same arithmetic as aes128_encrypt (FIPS-197 5.1, T-table form).
+struct RepAes {
+    uint32_t base;   // shared-memory byte address of the tables + 4 * lane
+    uint32_t c128;   // = 128, opaque to the compiler
+};
+template <int BYTE, int TABLE>
+__device__ __forceinline__ uint32_t rep_lookup(const RepAes &A, uint32_t word) {
+    const uint32_t b = __byte_perm(word, 0u, 0x4440 + BYTE);
+    uint32_t addr, v;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(addr) : "r"(b), "r"(A.c128), "r"(A.base));
+    asm("ld.shared.u32 %0, [%1 + %2];" : "=r"(v) : "r"(addr), "n"(TABLE * 32768));
+    return v;
 }
 template <typename RkPtr>
-__device__ __forceinline__ void aes128_encrypt_rep32(const char *tab, uint32_t lane4, const RkPtr rk, uint32_t (&s)[4]) {
+__device__ __forceinline__ void aes128_encrypt_rep32(const RepAes &A, const RkPtr rk, uint32_t (&s)[4]) {
     uint32_t s0 = s[0] ^ rk[0], s1 = s[1] ^ rk[1], s2 = s[2] ^ rk[2], s3 = s[3] ^ rk[3];
 #pragma unroll
     for (int r = 1; r < 10; ++r) {
-        const uint32_t t0 = rep_lookup(tab, s0, 0, 0, lane4) ^ rep_lookup(tab, s1, 1, 1, lane4) ^ rep_lookup(tab, s2, 2, 2, lane4) ^
-                            rep_lookup(tab, s3, 3, 3, lane4) ^ rk[4 * r + 0];
-        const uint32_t t1 = rep_lookup(tab, s1, 0, 0, lane4) ^ rep_lookup(tab, s2, 1, 1, lane4) ^ rep_lookup(tab, s3, 2, 2, lane4) ^
-                            rep_lookup(tab, s0, 3, 3, lane4) ^ rk[4 * r + 1];
-        const uint32_t t2 = rep_lookup(tab, s2, 0, 0, lane4) ^ rep_lookup(tab, s3, 1, 1, lane4) ^ rep_lookup(tab, s0, 2, 2, lane4) ^
-                            rep_lookup(tab, s1, 3, 3, lane4) ^ rk[4 * r + 2];
-        const uint32_t t3 = rep_lookup(tab, s3, 0, 0, lane4) ^ rep_lookup(tab, s0, 1, 1, lane4) ^ rep_lookup(tab, s1, 2, 2, lane4) ^
-                            rep_lookup(tab, s2, 3, 3, lane4) ^ rk[4 * r + 3];
+        const uint32_t t0 = rep_lookup<0, 0>(A, s0) ^ rep_lookup<1, 1>(A, s1) ^ rep_lookup<2, 2>(A, s2) ^ rep_lookup<3, 3>(A, s3) ^ rk[4 * r + 0];
+        const uint32_t t1 = rep_lookup<0, 0>(A, s1) ^ rep_lookup<1, 1>(A, s2) ^ rep_lookup<2, 2>(A, s3) ^ rep_lookup<3, 3>(A, s0) ^ rk[4 * r + 1];
+        const uint32_t t2 = rep_lookup<0, 0>(A, s2) ^ rep_lookup<1, 1>(A, s3) ^ rep_lookup<2, 2>(A, s0) ^ rep_lookup<3, 3>(A, s1) ^ rk[4 * r + 2];
+        const uint32_t t3 = rep_lookup<0, 0>(A, s3) ^ rep_lookup<1, 1>(A, s0) ^ rep_lookup<2, 2>(A, s1) ^ rep_lookup<3, 3>(A, s2) ^ rk[4 * r + 3];
         s0 = t0; s1 = t1; s2 = t2; s3 = t3;
     }
     // final round: SubBytes + ShiftRows. S sits in byte 0 of T2, bytes 1 and 2 of T0 and byte 3 of T1 (T0 = (2S, S, S, 3S)).
-#define FEDS_LAST(a, b, c, d)                                                                                                    \
-    __byte_perm(__byte_perm(rep_lookup(tab, a, 0, 2, lane4), rep_lookup(tab, b, 1, 0, lane4), 0x3250),                            \
-                __byte_perm(rep_lookup(tab, c, 2, 0, lane4), rep_lookup(tab, d, 3, 1, lane4), 0x7210), 0x7610)
+#define FEDS_LAST(a, b, c, d)                                                                       \
+    __byte_perm(__byte_perm(rep_lookup<0, 2>(A, a), rep_lookup<1, 0>(A, b), 0x3250),                 \
+                __byte_perm(rep_lookup<2, 0>(A, c), rep_lookup<3, 1>(A, d), 0x7210), 0x7610)
     const uint32_t u0 = FEDS_LAST(s0, s1, s2, s3), u1 = FEDS_LAST(s1, s2, s3, s0), u2 = FEDS_LAST(s2, s3, s0, s1), u3 = FEDS_LAST(s3, s0, s1, s2);
 #undef FEDS_LAST
     s[0] = u0 ^ rk[40]; s[1] = u1 ^ rk[41]; s[2] = u2 ^ rk[42]; s[3] = u3 ^ rk[43];
@@ -267,8 +270,9 @@ __global__ void __launch_bounds__(AES_THREADS) aes_ctr_stream_kernel(const __gri
     }
     ReplTable<REPL> T;
     T.b = sTab + (REPL > 1 ? (threadIdx.x & (REPL - 1)) : 0);
-    const char *tabb = reinterpret_cast<const char *>(sTab);
-    const uint32_t lane4 = 4u * (threadIdx.x & 31);
+    RepAes A;
+    A.base = (uint32_t)__cvta_generic_to_shared(sTab) + 4u * (threadIdx.x & 31);
+    A.c128 = p.c128;
     const unsigned long long nfull = p.n_bytes >> 4;
     const unsigned long long stride = (unsigned long long)gridDim.x * AES_THREADS;
     const unsigned long long total = nfull * p.n_msgs;
@@ -281,7 +285,7 @@ __global__ void __launch_bounds__(AES_THREADS) aes_ctr_stream_kernel(const __gri
         uint4 v = __ldg(reinterpret_cast<const uint4 *>(p.in + (size_t)m * p.in_stride) + blk);
         uint32_t ks[4];
         ctr_block(nonce, blk, ks);
-        if (REPL == 32) aes128_encrypt_rep32(tabb, lane4, p.rk, ks); else aes128_encrypt(T, p.rk, ks);
+        if (REPL == 32) aes128_encrypt_rep32(A, p.rk, ks); else aes128_encrypt(T, p.rk, ks);
         v.x ^= ks[0]; v.y ^= ks[1]; v.z ^= ks[2]; v.w ^= ks[3];
         reinterpret_cast<uint4 *>(p.out + (size_t)m * p.out_stride)[blk] = v;
     }

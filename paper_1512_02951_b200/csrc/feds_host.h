@@ -19,13 +19,19 @@ feds_status cuda_fail(cudaError_t e);
 int sm_count();                       // SMs of the current device (the persistent kernels launch one CTA per SM)
 cudaEvent_t prof_start_event();       // thread-local profiling hook (feds_profile_events), or nullptr
 cudaEvent_t prof_stop_event();
+void count_launch();                  // + 1 on the calling thread's launch counter
 
 #define FEDS_CUDA(call)                                        \
     do {                                                       \
         cudaError_t e__ = (call);                              \
         if (e__ != cudaSuccess) return ::feds::cuda_fail(e__); \
     } while (0)
-#define FEDS_LAUNCH_CHECK() FEDS_CUDA(cudaGetLastError())
+// every kernel launch of the library goes through this: error check + the per-thread launch counter (feds_debug_launch_count)
+#define FEDS_LAUNCH_CHECK()             \
+    do {                                \
+        ::feds::count_launch();         \
+        FEDS_CUDA(cudaGetLastError()); \
+    } while (0)
 
 // cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per process and kernel instantiation: the attribute is a property of
 // the loaded function, not data state of a call (a `static bool` per instantiation; racing first calls set the same value).
@@ -37,20 +43,19 @@ inline feds_status set_smem_once(K kernel, size_t bytes, size_t &done_bytes) {
     return FEDS_OK;
 }
 
-// ---- feds_k_dct_fused.cu: thread-per-leaf fused fragment kernel (steps 1-5), V in {2, 4}
+// ---- feds_k_dct_fused.cu: warp-specialised fused kernels (steps 1-5 / 6-8 with verification): bulk-copy tile groups + hash warps
+bool dct_fused_supported(const DctParams &p, int c);
 feds_status launch_fragment_fused(const DctParams &p, int c, cudaStream_t stream);
-// ---- feds_k_dct_ws.cu: warp-specialised fused kernels (steps 1-5 / 6-8 with verification)
-bool dct_ws_supported(const DctParams &p, int c);
-feds_status launch_fragment_ws(const DctParams &p, int c, cudaStream_t stream);
-feds_status launch_defragment_ws(const DctParams &p, int c, cudaStream_t stream);
+feds_status launch_defragment_fused(const DctParams &p, int c, cudaStream_t stream);
 // ---- feds_k_dct_tma.cu: the digest-free tile kernels on bulk asynchronous copies (w % 32 == 0 and at least one tile per block row)
 bool dct_tma_supported(const DctParams &p, int c);
-feds_status launch_fragment_tma(const DctParams &p, int c, cudaStream_t stream);
-feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream, bool record_start);
+feds_status launch_fragment_tma(const DctParams &p, int c, cudaStream_t stream, bool profile);
+feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream, bool profile);
 // ---- feds_k_dct_tile.cu: digest-free tile kernels and the registers-only leaf-hash kernel
-feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream);
-feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t stream, bool record_start);
-feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream);
+// (`profile`: record the thread's profiling events, if any, around this kernel -- the caller sets it for the dominant kernel of the call)
+feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream, bool profile);
+feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t stream, bool profile);
+feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream, bool profile);
 // ---- feds_k_hash.cu: Merkle upper levels, stream leaves, AES-CTR stream, digest compare
 feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
                      int skip_odd, cudaStream_t stream);

@@ -13,38 +13,38 @@ bool dct_tma_supported(const DctParams &p, int c) {
 
 namespace {
 template <int C, typename Kernel>
-feds_status launch_tma(Kernel kernel, const DctParams &p, cudaStream_t stream, bool record_start, size_t &smem_set) {
+feds_status launch_tma(Kernel kernel, const DctParams &p, cudaStream_t stream, bool profile, size_t &smem_set) {
     using S = TmaShape<C>;
     const size_t smem = tma_smem_bytes<C>(p.k, S::GROUPS);
     feds_status s = set_smem_once(kernel, smem, smem_set);
     if (s != FEDS_OK) return s;
     const unsigned long long tiles = (unsigned long long)p.n_images * (((unsigned long long)p.nbr * p.nbc + S::TB - 1) / S::TB);
     const unsigned grid = (unsigned)std::min<unsigned long long>((tiles + S::GROUPS - 1) / S::GROUPS, (unsigned long long)sm_count());
-    if (prof_start_event() && record_start) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
     kernel<<<grid, S::CTA, smem, stream>>>(p);
-    if (prof_stop_event()) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;
 }
-template <int C, int V> feds_status frag(const DctParams &p, cudaStream_t s) {
+template <int C, int V> feds_status frag(const DctParams &p, cudaStream_t s, bool profile) {
     static size_t smem_set = 0;
-    return launch_tma<C>(fragment_dct_tma_kernel<C, V>, p, s, true, smem_set);
+    return launch_tma<C>(fragment_dct_tma_kernel<C, V>, p, s, profile, smem_set);
 }
-template <int C, int V> feds_status defrag(const DctParams &p, cudaStream_t s, bool record_start) {
+template <int C, int V> feds_status defrag(const DctParams &p, cudaStream_t s, bool profile) {
     static size_t smem_set = 0;
-    return launch_tma<C>(defragment_dct_tma_kernel<C, V>, p, s, record_start, smem_set);
+    return launch_tma<C>(defragment_dct_tma_kernel<C, V>, p, s, profile, smem_set);
 }
 }  // namespace
 
-feds_status launch_fragment_tma(const DctParams &p, int c, cudaStream_t stream) {
+feds_status launch_fragment_tma(const DctParams &p, int c, cudaStream_t stream, bool profile) {
     const int V = dct_vec_width(p.k);
-#define FEDS_V(CC) (V == 4 ? frag<CC, 4>(p, stream) : V == 2 ? frag<CC, 2>(p, stream) : frag<CC, 1>(p, stream))
+#define FEDS_V(CC) (V == 4 ? frag<CC, 4>(p, stream, profile) : V == 2 ? frag<CC, 2>(p, stream, profile) : frag<CC, 1>(p, stream, profile))
     return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
 #undef FEDS_V
 }
-feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream, bool record_start) {
+feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream, bool profile) {
     const int V = dct_vec_width(p.k);
-#define FEDS_V(CC) (V == 4 ? defrag<CC, 4>(p, stream, record_start) : V == 2 ? defrag<CC, 2>(p, stream, record_start) : defrag<CC, 1>(p, stream, record_start))
+#define FEDS_V(CC) (V == 4 ? defrag<CC, 4>(p, stream, profile) : V == 2 ? defrag<CC, 2>(p, stream, profile) : defrag<CC, 1>(p, stream, profile))
     return c == 1 ? FEDS_V(1) : c == 3 ? FEDS_V(3) : FEDS_V(4);
 #undef FEDS_V
 }

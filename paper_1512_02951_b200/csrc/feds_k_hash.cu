@@ -111,6 +111,7 @@ feds_status launch_aes_ctr(const uint8_t *d_in, size_t in_stride, uint8_t *d_out
     CtrParams cp{};
     cp.in = d_in; cp.out = d_out; cp.n_bytes = n_bytes; cp.in_stride = in_stride; cp.out_stride = out_stride; cp.n_msgs = n_msgs;
     cp.d_nonces = d_nonces;
+    cp.c128 = 128u;
     if (nonce_host) nonce_to_be(nonce_host, cp.nonce_be);
     aes128_expand_key_host(key, cp.rk, h_aes);
     const unsigned long long nblk = ((n_bytes + 15) / 16) * n_msgs;

@@ -396,12 +396,13 @@ def test_bulk_copy_and_generic_tile_kernels_agree(orc, b, n, w, h, c, k):
         assert torch.equal(out, d_imgs)
 
 
-# Steps 1-5 (and 6-8 with verification) run either in the warp-specialised fused kernels (feds_dct_ws.cuh: whole 8-block leaves,
-# k + 1 even) or as tile kernel + leaf-hash kernel (everything else); the library picks by shape and size, FEDS_FLAG_FORCE_FUSED /
-# FEDS_FLAG_FORCE_SPLIT override it. Both routes must produce the same bytes, digests, images and flags at any size.
-WS_CASES = [(1, 64, 8, 1, 3), (2, 256, 16, 3, 3), (1, 1024, 24, 1, 5), (3, 1920, 16, 3, 7), (2, 512, 40, 4, 1), (1, 2048, 8, 1, 9),
+# Steps 1-5 (and 6-8 with verification) run either as the digest-free tile kernel and the leaf-hash kernel one after the other (the
+# default: measured faster) or in ONE warp-specialised kernel (feds_dct_fused.cuh: bulk-copy tile groups + hash warps; needs
+# w % 64 == 0 and at least one tile per block row). FEDS_FLAG_FORCE_FUSED / FEDS_FLAG_FORCE_SPLIT pick the route. Both routes must
+# produce the same bytes, digests, images and flags at any size and any k.
+WS_CASES = [(1, 512, 8, 1, 3), (2, 256, 16, 3, 3), (1, 1024, 24, 1, 5), (3, 1920, 16, 3, 7), (2, 512, 40, 4, 1), (1, 2048, 8, 1, 9),
             (1, 256, 64, 3, 31), (1, 512, 8, 4, 61), (1, 2048, 8, 3, 63), (7, 1920, 136, 3, 3), (1, 4096, 264, 3, 5), (3, 2048, 72, 4, 3),
-            (2, 8192, 24, 1, 3), (40, 64, 64, 3, 3)]
+            (2, 8192, 24, 1, 3), (40, 256, 64, 3, 3), (2, 320, 24, 3, 4), (1, 576, 16, 1, 0), (2, 1920, 1080, 3, 2)]
 
 
 @pytest.mark.parametrize("n,w,h,c,k", WS_CASES)
@@ -450,10 +451,10 @@ def test_fused_and_split_routes_agree(orc, b, n, w, h, c, k):
 
 
 def test_forced_route_that_cannot_run_is_refused(b):
-    """FEDS_FLAG_FORCE_FUSED on a shape the fused kernels do not support (ragged last leaf: (w/8) % 8 != 0; odd k + 1) returns
+    """FEDS_FLAG_FORCE_FUSED on a shape the fused kernels do not support (ragged last leaf: (w/8) % 8 != 0; narrower than a tile) returns
     FEDS_ERR_BAD_PARAM before anything is enqueued; both force flags together likewise."""
     key, nonce = synth.key_nonce(1)
-    for (w, h, c, k) in [(520, 16, 3, 3), (512, 16, 3, 2)]:
+    for (w, h, c, k) in [(520, 16, 3, 3), (224, 16, 3, 3), (288, 16, 1, 3)]:
         img = torch.zeros((1, h, w, c), dtype=torch.uint8, device="cuda")
         non = torch.zeros((1, 16), dtype=torch.uint8, device="cuda")
         batch = b.DctBatch(1, w, h, c, k)

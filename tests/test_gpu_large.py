@@ -1,6 +1,6 @@
 """GPU parity at the large end of BASELINE configs[4] (the sweep): square images 8192^2 and 16384^2, DCT k in {0, 2, 5, 9} and
 DWT levels in {1, 2, 3, 4} -- SURVEY.md 8(d) row 5: "on larger sizes digests only". At these sizes a fragment is 0.8-4.2 GB, i.e.
-byte offsets pass 2^31 (RGB) and 2^32 (four channels, k = 0): exactly where a 32-bit index in a kernel would wrap.
+byte offsets pass 2^31 (RGB) and 2^32 (four channels, 16384 x 17408, k = 0): exactly where a 32-bit index in a kernel would wrap.
 
 DCT, per (size, k), in the launch configuration bench.py's sweep times (feds_fragment_dct / feds_defragment_dct, one image):
   * both digests: the oracle's Merkle root (orc_merkle_blocks) of the fragment bytes the GPU stored, bit-exact;
@@ -30,9 +30,9 @@ def b():
     return binding
 
 
-def _image(size, c, seed):
+def _image(w, h, c, seed):
     """The sweep's recipe generated in HBM (numpy would take minutes at 16384^2); the same bytes go to both sides."""
-    d = synth.image_batch_torch(1, size, size, c, seed=seed, device="cuda")[0].contiguous()
+    d = synth.image_batch_torch(1, w, h, c, seed=seed, device="cuda")[0].contiguous()
     return d, d.cpu().numpy()
 
 
@@ -54,9 +54,9 @@ def _check_crops(orc, img, priv, pub, k, key, nonce, crops):
                 assert np.abs(got - ref[ch, r]).max() <= TOL, (by, bx, ch, r)
 
 
-def _dct_size(orc, b, size, c, ks, seed):
-    w = h = size
-    d_img, img = _image(size, c, seed)
+def _dct_size(orc, b, size, c, ks, seed, h=None):
+    w, h = size, (h or size)
+    d_img, img = _image(w, h, c, seed)
     nbr, nbc = h // 8, w // 8
     rng = np.random.default_rng(size + c)
     crops = [(0, 0), (nbr - 8, nbc - 8)] + [(int(rng.integers(0, nbr - 8)), int(rng.integers(0, nbc - 8))) for _ in range(2)]
@@ -88,17 +88,17 @@ def test_sweep_large_dct(orc, b, size):
 
 
 def test_fragment_offsets_beyond_2_pow_32(orc, b):
-    """16384 x 16384 x 4 channels, k = 0: the public fragment is 4.23 GB, so byte offsets cross 2^31 and 2^32 inside one fragment
-    (and the private one, 67 MB, has 4.2 M counter blocks)."""
-    assert orc.dct_public_bytes(16384, 16384, 4, 0) > 1 << 32
-    _dct_size(orc, b, 16384, 4, [0], seed=77)
+    """16384 x 17408 x 4 channels, k = 0: the public fragment is 4.49 GB, so byte offsets cross 2^31 and 2^32 inside one fragment
+    (and the private one, 71 MB, has 4.5 M counter blocks)."""
+    assert orc.dct_public_bytes(16384, 17408, 4, 0) > 1 << 32
+    _dct_size(orc, b, 16384, 4, [0], seed=77, h=17408)
 
 
 @pytest.mark.parametrize("size", [8192, 16384])
 def test_sweep_large_dwt(orc, b, size):
     w = h = size
     c = 3
-    d_img, img = _image(size, c, seed=6000 + size)
+    d_img, img = _image(size, size, c, seed=6000 + size)
     with ThreadPoolExecutor(max_workers=4) as ex:
         futs = {}
         for L in [1, 2, 3, 4]:
