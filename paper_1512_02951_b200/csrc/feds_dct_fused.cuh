@@ -155,13 +155,13 @@ __device__ __forceinline__ void fu_fragment_tiles(const DctParams &p, const FuWo
     TmaTile T, Tn;
     unsigned s = (unsigned)gid;
     while (s < s_end && !fu_tile<C, TPU>(p, W, s, T)) s += NP;
-    if (s < s_end && tid == 0) tma_move_pixels<C, false>(p, T, smem_u32(G.pix[0]), G.bar[0]);
+    if (s < s_end && tid == TmaShape<C>::LOADER) tma_move_pixels<C, false>(p, T, smem_u32(G.pix[0]), G.bar[0]);
 #pragma unroll 1
     for (unsigned it = 0; s < s_end; ++it) {
         const int st = it & 1;
         unsigned sn = s + NP;
         while (sn < s_end && !fu_tile<C, TPU>(p, W, sn, Tn)) sn += NP;
-        if (tid == 0 && sn < s_end) tma_move_pixels<C, false>(p, Tn, smem_u32(G.pix[st ^ 1]), G.bar[st ^ 1]);
+        if (tid == TmaShape<C>::LOADER && sn < s_end) tma_move_pixels<C, false>(p, Tn, smem_u32(G.pix[st ^ 1]), G.bar[st ^ 1]);
         mbar_wait(G.bar[st], (it >> 1) & 1);
         tma_fragment_tile<C, V, true>(p, sT, G, T, G.pix[st], [&]() {
             if (tid == 0) {
@@ -188,14 +188,14 @@ __device__ __forceinline__ void fu_defragment_tiles(const DctParams &p, const Fu
     TmaTile T, Tn;
     unsigned s = (unsigned)gid;
     while (s < s_end && !fu_tile<C, TPU>(p, W, s, T)) s += NP;
-    if (s < s_end && tid == 0) tma_move_runs<C, false>(p, T, smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
+    if (s < s_end && tid == TmaShape<C>::LOADER) tma_move_runs<C, false>(p, T, smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
 #pragma unroll 1
     for (unsigned it = 0; s < s_end; ++it) {
         unsigned sn = s + NP;
         while (sn < s_end && !fu_tile<C, TPU>(p, W, sn, Tn)) sn += NP;
         mbar_wait(G.bar[0], it & 1);
         tma_defragment_tile<C, V, true>(p, sT, G, T, [&]() {
-            if (tid == 0 && sn < s_end) tma_move_runs<C, false>(p, Tn, smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
+            if (tid == TmaShape<C>::LOADER && sn < s_end) tma_move_runs<C, false>(p, Tn, smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
         });
         if (tid == 0) tma_move_pixels<C, true>(p, T, smem_u32(G.pix[1]), 0u);
         s = sn;

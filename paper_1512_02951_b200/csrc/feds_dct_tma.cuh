@@ -34,6 +34,9 @@ template <int C> struct TmaShape {
     static constexpr int CTA = THREADS * GROUPS;
     static constexpr int BLOCK_ROW_BYTES = 8 * C;        // one pixel row of one block, all channels
     static constexpr int PIX_BYTES = TB * 8 * BLOCK_ROW_BYTES;   // one pixel tile
+    // bulk loads are issued by lane 0 of the group's last warp, bulk stores by lane 0 of its first: the issuing warp runs ~150
+    // instructions per tile that the others do not, and every barrier waits for the slowest warp
+    static constexpr int LOADER = THREADS - 32;
 };
 constexpr int TMA_BAR_BYTES = 256;   // mbarriers of all groups (2 x 8 bytes each), behind the AES table
 
@@ -334,13 +337,13 @@ __global__ void __launch_bounds__(TmaShape<C>::CTA, 1) fragment_dct_tma_kernel(c
     const unsigned tiles_per_plane = ((unsigned)p.nbr * p.nbc + S::TB - 1) / S::TB;
     const unsigned total = (unsigned)p.n_images * tiles_per_plane, step = gridDim.x * S::GROUPS;
     unsigned t = blockIdx.x * S::GROUPS + gid;
-    if (t < total && tid == 0) tma_move_pixels<C, false>(p, tma_decode_tile<C>(p, t, tiles_per_plane), smem_u32(G.pix[0]), G.bar[0]);
+    if (t < total && tid == S::LOADER) tma_move_pixels<C, false>(p, tma_decode_tile<C>(p, t, tiles_per_plane), smem_u32(G.pix[0]), G.bar[0]);
 #pragma unroll 1
     for (unsigned it = 0; t < total; t += step, ++it) {
         const int s = it & 1;
         const TmaTile T = tma_decode_tile<C>(p, t, tiles_per_plane);
         // the other pixel tile was last read one iteration ago, before that iteration's barriers: refill it now
-        if (tid == 0 && t + step < total) tma_move_pixels<C, false>(p, tma_decode_tile<C>(p, t + step, tiles_per_plane), smem_u32(G.pix[s ^ 1]), G.bar[s ^ 1]);
+        if (tid == S::LOADER && t + step < total) tma_move_pixels<C, false>(p, tma_decode_tile<C>(p, t + step, tiles_per_plane), smem_u32(G.pix[s ^ 1]), G.bar[s ^ 1]);
         mbar_wait(G.bar[s], (it >> 1) & 1);
         tma_fragment_tile<C, V>(p, sT, G, T, G.pix[s], [&]() {
             if (tid == 0) bulk_wait_read0();   // the previous tile's stores have read the stage
@@ -457,13 +460,13 @@ __global__ void __launch_bounds__(TmaShape<C>::CTA, 1) defragment_dct_tma_kernel
     const unsigned tiles_per_plane = ((unsigned)p.nbr * p.nbc + S::TB - 1) / S::TB;
     const unsigned total = (unsigned)p.n_images * tiles_per_plane, step = gridDim.x * S::GROUPS;
     unsigned t = blockIdx.x * S::GROUPS + gid;
-    if (t < total && tid == 0) tma_move_runs<C, false>(p, tma_decode_tile<C>(p, t, tiles_per_plane), smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
+    if (t < total && tid == S::LOADER) tma_move_runs<C, false>(p, tma_decode_tile<C>(p, t, tiles_per_plane), smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
 #pragma unroll 1
     for (unsigned it = 0; t < total; t += step, ++it) {
         const TmaTile T = tma_decode_tile<C>(p, t, tiles_per_plane);
         mbar_wait(G.bar[0], it & 1);
         tma_defragment_tile<C, V>(p, sT, G, T, [&]() {
-            if (tid == 0 && t + step < total) tma_move_runs<C, false>(p, tma_decode_tile<C>(p, t + step, tiles_per_plane), smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
+            if (tid == S::LOADER && t + step < total) tma_move_runs<C, false>(p, tma_decode_tile<C>(p, t + step, tiles_per_plane), smem_u32(G.s_pub), G.RSQ, G.RSP, G.bar[0]);
         });
         if (tid == 0) tma_move_pixels<C, true>(p, T, smem_u32(G.pix[1]), 0u);
     }
