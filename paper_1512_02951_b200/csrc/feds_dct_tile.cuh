@@ -13,6 +13,7 @@
 //   were measured to cost a third of the kernel's time); T1..T3 are byte rotations of T0.
 #pragma once
 #include "feds_dct.cuh"
+#include "feds_sha_coop.cuh"
 
 namespace feds {
 
@@ -352,6 +353,49 @@ __global__ void __launch_bounds__(LEAFHASH_THREADS) dct_leaves_hash_kernel(const
     w[14] = (uint32_t)(bits >> 32); w[15] = (uint32_t)bits;
     sha256_compress_rolled_fma(H, w, p.one);
     store_digest(p.leaves + (((size_t)L.n * 2 + (priv ? 0 : 1)) * p.leaves_per_image + L.li) * 32, H);
+}
+
+// The same digests for SMALL inputs, where what counts is the latency of one leaf's chain of compressions and not throughput:
+// one WARP per public leaf (sha256_warp_coop, feds_sha_coop.cuh: ~23 us for 31 compressions instead of ~60), the short private
+// leaves one per thread behind them. The host takes this kernel while there are at most COOP_MAX_LEAVES public leaves: one
+// cooperating warp per warp scheduler of the chip (more would share the ALU pipes: measured slower from two per scheduler on).
+constexpr int COOP_WARPS = 4, COOP_STRIDE = 32;
+constexpr unsigned COOP_MAX_LEAVES = 592;
+constexpr size_t COOP_SMEM_BYTES = (size_t)COOP_WARPS * coop_ws_words<COOP_STRIDE>() * 4;
+template <int C>
+__global__ void __launch_bounds__(COOP_WARPS * 32) dct_leaves_hash_coop_kernel(const __grid_constant__ DctParams p) {
+    extern __shared__ __align__(16) uint32_t coop_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const unsigned long long wid = (unsigned long long)blockIdx.x * COOP_WARPS + warp;
+    const int P = p.k + 1, Q = 63 - p.k;
+    if (wid < p.total_leaves) {   // a public leaf, by the whole warp
+        if (Q == 0) return;
+        const LeafCoord L = decode_leaf<C>(p, wid);
+        const uint8_t *src = p.pub + (size_t)L.n * p.pub_stride + (size_t)L.b0 * Q * 4;
+        uint32_t H[8];
+        sha256_warp_coop<COOP_STRIDE>(src, (unsigned)(L.nblk * Q) * 4u, coop_smem + warp * coop_ws_words<COOP_STRIDE>(), lane, p.one, H);
+        if (lane == 0) store_digest(p.leaves + (((size_t)L.n * 2 + 1) * p.leaves_per_image + L.li) * 32, H);
+        return;
+    }
+    // 32 private leaves, one per lane
+    const unsigned long long gid = (wid - p.total_leaves) * 32 + lane;
+    if (gid >= p.total_leaves) return;
+    const LeafCoord L = decode_leaf<C>(p, gid);
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
+    const unsigned nwords = (unsigned)(L.nblk * P), nblocks = (nwords * 4u + 9u + 63u) / 64u;
+    uint32_t H[8], w[16];
+    sha256_init(H);
+#pragma unroll 1
+    for (unsigned i = 0; i < nblocks; ++i) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const unsigned idx = 16u * i + j;
+            w[j] = idx < nwords ? bswap32(__ldg(src + idx)) : (idx == nwords ? 0x80000000u : 0u);
+        }
+        if (i == nblocks - 1) w[15] = nwords * 32u;
+        sha256_compress_rolled_fma(H, w, p.one);
+    }
+    store_digest(p.leaves + (((size_t)L.n * 2 + 0) * p.leaves_per_image + L.li) * 32, H);
 }
 
 }  // namespace feds

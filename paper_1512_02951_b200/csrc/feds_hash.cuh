@@ -3,6 +3,7 @@
 #pragma once
 #include "feds_device.cuh"
 #include "feds_dct.cuh"  // g_aes, load_aes_tables, store_digest
+#include "feds_sha_coop.cuh"
 
 namespace feds {
 
@@ -82,34 +83,49 @@ __global__ void __launch_bounds__(HASH_THREADS) merkle_level_kernel(const __grid
 }
 
 // The top of a tree in one launch: one CTA per tree reduces n_in <= 4096 digests to the root (up to three levels of
-// fan-out 16: <= 256 nodes, <= 16 nodes, 1), intermediate levels in shared memory.
-constexpr int TAIL_THREADS = 256;
-constexpr unsigned TAIL_MAX_IN = TAIL_THREADS * FANOUT;
+// fan-out 16: <= 256 nodes, <= 16 nodes, 1), intermediate levels in shared memory. The levels run one after the other on a
+// nearly empty SM, so what counts is the length of the dependent chain: a level with more than TAIL_WARPS nodes is hashed one
+// node per thread (nine dependent compressions, ~18 us), a level with at most TAIL_WARPS nodes one node per WARP, each warp on
+// its own scheduler (sha256_warp_coop: the nine message schedules side by side, then 9 x 64 short rounds, ~6 us). More
+// cooperating warps than schedulers would share the ALU pipes and lose again (measured: 32 warps, 47 us).
+constexpr int TAIL_THREADS = 256, TAIL_WARPS = 4, TAIL_STRIDE = 16;   // TAIL_WARPS: one cooperating warp per warp scheduler; a node is at most 9 blocks
+constexpr unsigned TAIL_MAX_IN = 256 * FANOUT;
+constexpr size_t TAIL_SMEM_BYTES = (size_t)(256 * 2 + FANOUT * 2) * 16 + (size_t)TAIL_WARPS * coop_ws_words<TAIL_STRIDE>() * 4;
 __global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_constant__ MerkleLevelParams p) {
-    __shared__ uint4 sA[TAIL_THREADS * 2];
-    __shared__ uint4 sB[FANOUT * 2];
-    const unsigned t = blockIdx.x, tid = threadIdx.x;
+    extern __shared__ __align__(16) uint4 tail_smem[];
+    uint4 *sA = tail_smem, *sB = tail_smem + 256 * 2;
+    uint32_t *ws = reinterpret_cast<uint32_t *>(sB + FANOUT * 2) + (threadIdx.x >> 5) * coop_ws_words<TAIL_STRIDE>();
+    const unsigned t = blockIdx.x, tid = threadIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool extra = t >= p.n_trees;
     if (!extra && p.odd_trees_only_if_nonempty && (t & 1u)) return;
     const unsigned t2 = extra ? t - p.n_trees : 0u;
     uint4 *root = reinterpret_cast<uint4 *>(extra ? p.out2 + (size_t)t2 * p.out2_tree_stride : p.out + (size_t)t * p.out_tree_stride);
-    // One hash_children call site serves all (up to three) levels: the levels run one after the other on a nearly empty SM,
-    // so what counts is the length of the dependent chain and the amount of cold code, not throughput. Level sources and
-    // sinks are generic pointers (global input, then the two shared buffers).
+    // Level sources and sinks are generic pointers (global input, then the two shared buffers).
     const uint4 *src = reinterpret_cast<const uint4 *>(extra ? p.in2 + (size_t)t2 * p.in2_tree_stride : p.in + (size_t)t * p.in_tree_stride);
     unsigned n = extra ? p.n_in2 : p.n_in;
     uint4 *dst = sA;
 #pragma unroll 1
     for (int level = 0; level < 3; ++level) {
         const unsigned m = (n + FANOUT - 1) / FANOUT;
-        if (tid < m) {
-            const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n) - lo;
-            uint32_t H[8];
-            hash_children<false>(src + 2 * (size_t)lo, cnt, H, p.one);
+        uint32_t H[8];
+        bool mine = false;
+        unsigned node = 0;
+        if (m > (unsigned)TAIL_WARPS) {
+            if (tid < m) {
+                const unsigned lo = tid * FANOUT, cnt = min(lo + FANOUT, n) - lo;
+                hash_children<false>(src + 2 * (size_t)lo, cnt, H, p.one);
+                mine = true; node = tid;
+            }
+        } else if (warp < m) {
+            const unsigned lo = warp * FANOUT, cnt = min(lo + FANOUT, n) - lo;
+            sha256_warp_coop<TAIL_STRIDE>(reinterpret_cast<const uint8_t *>(src + 2 * (size_t)lo), cnt * 32u, ws, (int)lane, p.one, H);
+            mine = lane == 0; node = warp;
+        }
+        if (mine) {
             uint4 a, b;
             digest_to_words(H, a, b);
             if (m == 1) { root[0] = a; root[1] = b; }
-            else { dst[2 * tid] = a; dst[2 * tid + 1] = b; }
+            else { dst[2 * node] = a; dst[2 * node + 1] = b; }
         }
         if (m == 1) return;
         __syncthreads();
@@ -188,6 +204,27 @@ __global__ void __launch_bounds__(LEAF_THREADS) stream_leaves_kernel(const __gri
         sha256_compress_rolled_fma(H, w, p.one);
     }
     store_digest(p.out[f] + ((size_t)img * p.n_leaves[f] + j) * 32, H);
+}
+
+// The same leaves for SHORT streams (at most STREAM_COOP_MAX leaves in the launch): one warp per leaf, sha256_warp_coop.
+constexpr int STREAM_COOP_WARPS = 4, STREAM_COOP_STRIDE = 32;
+constexpr unsigned STREAM_COOP_MAX = 592;   // one warp per warp scheduler of the chip: more would share the ALU pipes and lose
+constexpr size_t STREAM_COOP_SMEM_BYTES = (size_t)STREAM_COOP_WARPS * coop_ws_words<STREAM_COOP_STRIDE>() * 4;
+__global__ void __launch_bounds__(STREAM_COOP_WARPS * 32) stream_leaves_coop_kernel(const __grid_constant__ StreamLeavesParams p) {
+    extern __shared__ __align__(16) uint32_t coop_smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const unsigned long long gid0 = (unsigned long long)blockIdx.x * STREAM_COOP_WARPS + warp;
+    const unsigned per_image = p.n_leaves[0] + p.n_leaves[1];
+    if (gid0 >= (unsigned long long)per_image * p.n_images) return;
+    const unsigned img = (unsigned)(gid0 / per_image), gid = (unsigned)(gid0 % per_image);
+    const int f = gid >= p.n_leaves[0] ? 1 : 0;
+    const unsigned j = f ? gid - p.n_leaves[0] : gid;
+    const unsigned long long lo = (unsigned long long)j * DWT_LEAF_BYTES;
+    const unsigned len = (unsigned)min((unsigned long long)DWT_LEAF_BYTES, p.n_bytes[f] - lo);
+    uint32_t H[8];
+    sha256_warp_coop<STREAM_COOP_STRIDE>(p.data[f] + (size_t)img * p.data_stride[f] + lo, len, coop_smem + warp * coop_ws_words<STREAM_COOP_STRIDE>(), lane,
+                                         p.one, H);
+    if (lane == 0) store_digest(p.out[f] + ((size_t)img * p.n_leaves[f] + j) * 32, H);
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -50,8 +50,21 @@ feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t strea
 // leaf digests of fragments as they lie in memory: the verification half of a verified defragment
 feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream, bool profile) {
     const unsigned long long threads = 2 * p.total_leaves;
-    const unsigned grid = (unsigned)((threads + LEAFHASH_THREADS - 1) / LEAFHASH_THREADS);
     if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (p.total_leaves <= COOP_MAX_LEAVES) {   // few leaves: a warp per public leaf shortens the chain of dependent compressions
+        static size_t smem_set[3] = {0, 0, 0};
+        const unsigned long long cwarps = p.total_leaves + (p.total_leaves + 31) / 32;   // public leaves + private leaves by 32
+        const unsigned cgrid = (unsigned)((cwarps + COOP_WARPS - 1) / COOP_WARPS);
+        feds_status s = FEDS_OK;
+        if (c == 1) { s = set_smem_once(dct_leaves_hash_coop_kernel<1>, COOP_SMEM_BYTES, smem_set[0]); if (s == FEDS_OK) dct_leaves_hash_coop_kernel<1><<<cgrid, COOP_WARPS * 32, COOP_SMEM_BYTES, stream>>>(p); }
+        else if (c == 3) { s = set_smem_once(dct_leaves_hash_coop_kernel<3>, COOP_SMEM_BYTES, smem_set[1]); if (s == FEDS_OK) dct_leaves_hash_coop_kernel<3><<<cgrid, COOP_WARPS * 32, COOP_SMEM_BYTES, stream>>>(p); }
+        else { s = set_smem_once(dct_leaves_hash_coop_kernel<4>, COOP_SMEM_BYTES, smem_set[2]); if (s == FEDS_OK) dct_leaves_hash_coop_kernel<4><<<cgrid, COOP_WARPS * 32, COOP_SMEM_BYTES, stream>>>(p); }
+        if (s != FEDS_OK) return s;
+        if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+        FEDS_LAUNCH_CHECK();
+        return FEDS_OK;
+    }
+    const unsigned grid = (unsigned)((threads + LEAFHASH_THREADS - 1) / LEAFHASH_THREADS);
     if (c == 1) dct_leaves_hash_kernel<1><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);
     else if (c == 3) dct_leaves_hash_kernel<3><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);
     else dct_leaves_hash_kernel<4><<<grid, LEAFHASH_THREADS, 0, stream>>>(p);

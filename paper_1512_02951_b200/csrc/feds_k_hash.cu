@@ -15,6 +15,11 @@ void nonce_to_be(const uint8_t nonce[16], uint32_t out[4]) {
         out[i] = ((uint32_t)nonce[4 * i] << 24) | ((uint32_t)nonce[4 * i + 1] << 16) | ((uint32_t)nonce[4 * i + 2] << 8) | nonce[4 * i + 3];
 }
 
+feds_status tail_smem_once() {
+    static size_t smem_set = 0;
+    return set_smem_once(merkle_tail_kernel, TAIL_SMEM_BYTES, smem_set);
+}
+
 // wide levels of n_trees equal trees: one thread per node until at most TAIL_MAX_IN digests per tree remain
 feds_status reduce_wide(const uint8_t *&in, unsigned &n, unsigned n_trees, uint8_t *&sc, int skip_odd, cudaStream_t stream) {
     MerkleLevelParams mp{};
@@ -50,7 +55,9 @@ feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8
         mp.n_trees = n_trees; mp.odd_trees_only_if_nonempty = skip_odd; mp.one = 1u;
         mp.in = in; mp.n_in = n; mp.n_out = 1; mp.in_tree_stride = (size_t)n * 32;
         mp.out = roots; mp.out_tree_stride = root_stride;
-        merkle_tail_kernel<<<n_trees, TAIL_THREADS, 0, stream>>>(mp);
+        feds_status ts = tail_smem_once();
+        if (ts != FEDS_OK) return ts;
+        merkle_tail_kernel<<<n_trees, TAIL_THREADS, TAIL_SMEM_BYTES, stream>>>(mp);
         FEDS_LAUNCH_CHECK();
     }
     return FEDS_OK;
@@ -81,7 +88,9 @@ feds_status run_two_trees(const uint8_t *l0a, unsigned na, uint8_t *sca, uint8_t
         }
         ctas += n_trees;
     }
-    merkle_tail_kernel<<<ctas, TAIL_THREADS, 0, stream>>>(mp);
+    feds_status ts = tail_smem_once();
+    if (ts != FEDS_OK) return ts;
+    merkle_tail_kernel<<<ctas, TAIL_THREADS, TAIL_SMEM_BYTES, stream>>>(mp);
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;
 }
@@ -98,6 +107,12 @@ feds_status launch_stream_leaves(const uint8_t *const d[2], const size_t stride[
     const unsigned long long total = (unsigned long long)(nl[0] + nl[1]) * n_images;
     if (total == 0) return FEDS_OK;
     if (profile && prof_start_event()) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (total <= STREAM_COOP_MAX) {   // few leaves: a warp per leaf shortens the chain of dependent compressions
+        static size_t smem_set = 0;
+        feds_status s = set_smem_once(stream_leaves_coop_kernel, STREAM_COOP_SMEM_BYTES, smem_set);
+        if (s != FEDS_OK) return s;
+        stream_leaves_coop_kernel<<<(unsigned)((total + STREAM_COOP_WARPS - 1) / STREAM_COOP_WARPS), STREAM_COOP_WARPS * 32, STREAM_COOP_SMEM_BYTES, stream>>>(sp);
+    } else
     stream_leaves_kernel<<<(unsigned)((total + LEAF_THREADS - 1) / LEAF_THREADS), LEAF_THREADS, 0, stream>>>(sp);
     if (profile && prof_stop_event()) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
     FEDS_LAUNCH_CHECK();

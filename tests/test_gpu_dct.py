@@ -489,3 +489,56 @@ def test_device_dct_bits_equal_the_host_build(orc, b):
         out = np.empty(64, dtype=np.float32)
         b.lib.feds_debug_dct8x8_host(x.ctypes.data, out.ctypes.data, 0)
         assert (out[zz].view(np.uint32) == coef[br, bc].view(np.uint32)).all()
+
+
+def test_cuda_graph_capture_and_replay(orc, b):
+    """The library allocates nothing, keeps no state and never synchronises (include/feds.h), so a fragment + verified defragment
+    pair -- DCT and DWT -- can be captured into a CUDA graph once and replayed on new pixels: the replays' fragments and digests are
+    the ones a direct call produces, bit for bit (and the direct call's are the oracle's, as every other test here checks)."""
+    n, w, h, c, k, L = 2, 512, 64, 3, 3, 2
+    key, nonce = synth.key_nonce(77)
+    nonces = synth.batch_nonces(nonce, n)
+    d_non = torch.from_numpy(nonces).cuda()
+    imgs = [torch.from_numpy(np.stack([synth.image(w, h, c, seed=900 + 10 * r + i) for i in range(n)])).cuda() for r in range(3)]
+    d_in = imgs[0].clone()
+    d_out, d_out2 = torch.zeros_like(d_in), torch.zeros_like(d_in)
+    dct, dwt = b.DctBatch(n, w, h, c, k), b.DwtBatch(n, w, h, c, L)
+
+    def work():
+        dct.fragment(d_in, key, d_non)
+        dct.defragment(d_out, key, d_non, expected=dct.digests)
+        dwt.fragment(d_in, key, d_non)
+        dwt.defragment(d_out2, key, d_non, expected=dwt.digests)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        work()                                   # first calls set kernel attributes: keep them out of the capture
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        work()
+    ref_dct, ref_dwt = b.DctBatch(n, w, h, c, k), b.DwtBatch(n, w, h, c, L)
+    for r in (1, 2, 0):
+        d_in.copy_(imgs[r])
+        for t in (dct.priv, dct.pub, dct.digests, dwt.priv, dwt.pub, dwt.digests, d_out, d_out2):
+            t.zero_()
+        dct.flags_out.fill_(7); dwt.flags_out.fill_(7)
+        graph.replay()
+        torch.cuda.synchronize()
+        ref_dct.fragment(imgs[r], key, d_non)
+        ref_dwt.fragment(imgs[r], key, d_non)
+        torch.cuda.synchronize()
+        assert torch.equal(dct.priv, ref_dct.priv) and torch.equal(dct.pub, ref_dct.pub) and torch.equal(dct.digests, ref_dct.digests)
+        assert torch.equal(dwt.priv, ref_dwt.priv) and torch.equal(dwt.pub, ref_dwt.pub) and torch.equal(dwt.digests, ref_dwt.digests)
+        assert torch.equal(d_out, imgs[r]) and torch.equal(d_out2, imgs[r])
+        assert int(dct.flags_out.abs().sum().item()) == 0 and int(dwt.flags_out.abs().sum().item()) == 0
+    # the replayed fragments are the oracle's for image 0 of the last round
+    pv = dct.priv[:dct.priv_bytes].cpu().numpy()
+    pb = dct.pub[:dct.pub_bytes].cpu().numpy()
+    coef = gpu_coefficients(orc, pv, pb, w * h * c // 64, k, key, nonces[0].tobytes())
+    p2, q2, d2 = orc.fragment_from_coef32(coef, w, h, c, k, key, nonces[0].tobytes())
+    assert (p2 == pv).all() and (q2 == pb).all() and d2 == dct.digests[:64].cpu().numpy().tobytes()
+    op, oq, odg = orc.fragment_dwt(imgs[0][0].cpu().numpy(), L, key, nonces[0].tobytes())
+    assert (dwt.priv[:dwt.priv_bytes].cpu().numpy() == op).all() and dwt.digests[:64].cpu().numpy().tobytes() == odg
