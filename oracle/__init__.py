@@ -250,3 +250,72 @@ def defragment_dwt(priv, pub, w, h, c, levels, key, nonce, expected=None, leaf_b
     if rc != 0:
         raise ValueError("orc_defragment_dwt rc=%d" % rc)
     return out, flags.value
+
+
+# ------------------------------------------------------------------------------------------ strong level (feds_oracle_strong.c)
+def sha512(msg) -> bytes:
+    a, p = _u8(np.frombuffer(bytes(msg), dtype=np.uint8))
+    out = (C.c_uint8 * 64)()
+    lib().orc_sha512(p, C.c_uint64(a.size), out)
+    return bytes(out)
+
+
+def strong_basis() -> np.ndarray:
+    """B[z][p] = rne(4096 b_z(p)), int32 [64][64]"""
+    out = np.zeros((64, 64), dtype=np.int32)
+    lib().orc_strong_basis(out.ctypes.data_as(C.POINTER(C.c_int32)))
+    return out
+
+
+def strong_public_bytes(w, h, c):
+    return w * h * c
+
+
+def fragment_dct_strong(image, k, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    """image -> (private ciphertext, public uint8 [block][64], digests[64]) at the strong level of protection"""
+    img, h, w, c = _img(image)
+    pi = img.ctypes.data_as(C.POINTER(C.c_uint8))
+    priv = np.zeros(dct_private_bytes(w, h, c, k), dtype=np.uint8)
+    pub = np.zeros(w * h * c, dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_dct_strong(pi, w, h, c, k, _key(key), _key(nonce), g, fanout, priv.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                       pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    assert rc == 0, rc
+    return priv, pub, bytes(dg)
+
+
+def fragment_strong_from_priv32(image, priv32, k, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    """stage (ii): everything after the DCT from given float32 private coefficients priv32[b][z <= k]"""
+    img, h, w, c = _img(image)
+    pi = img.ctypes.data_as(C.POINTER(C.c_uint8))
+    p32 = np.ascontiguousarray(priv32, dtype=np.float32)
+    assert p32.size == (w // 8) * (h // 8) * c * (k + 1)
+    priv = np.zeros(dct_private_bytes(w, h, c, k), dtype=np.uint8)
+    pub = np.zeros(w * h * c, dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_strong_from_priv32(pi, p32.ctypes.data_as(C.POINTER(C.c_float)), w, h, c, k, _key(key), _key(nonce), g, fanout,
+                                               priv.ctypes.data_as(C.POINTER(C.c_uint8)), pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    assert rc == 0, rc
+    return priv, pub, bytes(dg)
+
+
+def defragment_dct_strong(priv, pub, w, h, c, k, key, nonce, expected=None, g=G_BLOCKS, fanout=FANOUT):
+    pa, pp = _u8(priv)
+    qa, qp = _u8(pub)
+    out = np.zeros((h, w, c), dtype=np.uint8)
+    fl = C.c_uint32(0)
+    exp = (C.c_uint8 * 64).from_buffer_copy(bytes(expected)) if expected is not None else None
+    rc = lib().orc_defragment_dct_strong(pp, qp, w, h, c, k, _key(key), _key(nonce), g, fanout, exp,
+                                         out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(fl))
+    assert rc == 0, rc
+    return out, int(fl.value)
+
+
+def strong_remainder(image, k) -> np.ndarray:
+    """x - L per pixel (signed, before the reduction modulo 256): int16 [h][w][c]"""
+    img, h, w, c = _img(image)
+    pi = img.ctypes.data_as(C.POINTER(C.c_uint8))
+    out = np.zeros((h, w, c), dtype=np.int16)
+    rc = lib().orc_strong_remainder(pi, w, h, c, k, out.ctypes.data_as(C.POINTER(C.c_int16)))
+    assert rc == 0, rc
+    return out
