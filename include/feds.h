@@ -111,6 +111,37 @@ feds_status feds_verify_dct_batch(const uint8_t *d_private, size_t private_strid
                                   size_t workspace_bytes, feds_stream_t stream);
 
 /*
+ * Strong level of protection (PAPER.md 6.3.2, Figure 8; byte format: DESIGN.md 2.3). Part 1 of every 8x8 block (DC +
+ * first k zigzag AC, float32) is encrypted with AES-128-CTR exactly as by feds_fragment_dct; the public part of a block is its
+ * 64 remainder pixels -- "the reverse DCT result of the rest DCT coefficients padded with zero", i.e. x minus the low-pass
+ * image of Part 1, evaluated in exact fixed-point arithmetic and stored modulo 256 -- XORed with SHA-512(Part 1 of the block)
+ * (one 512-bit string per block). Digests: the Merkle roots of the two fragments as stored, as everywhere else.
+ *   d_public: feds_dct_strong_public_bytes(w,h,c) = w*h*c bytes, uint8 [block][64], blocks in the order of feds_fragment_dct.
+ *   d_private, d_digests, workspace (feds_workspace_bytes(w,h,c,k,0)), key, nonce, errors: as feds_fragment_dct.
+ * The inverse rebuilds the low-pass image and the keystream from the decrypted Part 1 and is exact (uint8 for uint8) by
+ * construction. *_batch: n_images images at the given byte strides, per-image nonces on the device; flags: FEDS_FLAG_NO_DIGEST.
+ */
+size_t feds_dct_strong_public_bytes(int w, int h, int c);
+feds_status feds_fragment_dct_strong(const uint8_t *d_image, int w, int h, int c, int k, const uint8_t key[16],
+                                     const uint8_t nonce[16], uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests,
+                                     void *d_workspace, size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_defragment_dct_strong(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k,
+                                       const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                       uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
+                                       size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_fragment_dct_strong_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c,
+                                           int k, const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private,
+                                           size_t private_stride, uint8_t *d_public, size_t public_stride,
+                                           uint8_t *d_digests, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                           feds_stream_t stream);
+feds_status feds_defragment_dct_strong_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public,
+                                             size_t public_stride, int n_images, int w, int h, int c, int k,
+                                             const uint8_t key[16], const uint8_t *d_nonces,
+                                             const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                             uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                                             unsigned flags, feds_stream_t stream);
+
+/*
  * feds_fragment_dwt / feds_defragment_dwt — rows D1-D8: level shift -128, `levels`-level whole-image
  * Le Gall 5/3 integer lifting, rows then columns, LL_levels -> private under AES-128-CTR,
  * the other subbands -> public (order: channel, level L..1, HL, LH, HH, row-major int16 LE), SHA-256 Merkle

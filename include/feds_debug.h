@@ -24,6 +24,7 @@ void feds_debug_sha256_host(const uint8_t *msg, size_t n, uint8_t out[32]);
 void feds_debug_aes128_host(const uint8_t key[16], const uint8_t in[16], uint8_t out[16]);
 void feds_debug_dct8x8_host(const float in[64], float out[64], int inverse);
 void feds_debug_zigzag_host(int out[64]);
+void feds_debug_strong_basis_host(int32_t out[64 * 64]); /* the strong level's fixed-point DCT basis B[z][p] */
 unsigned long long feds_debug_launch_count(void);
 
 #ifdef __cplusplus

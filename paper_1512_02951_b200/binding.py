@@ -31,6 +31,8 @@ SYMBOLS = [
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
     "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
+    "feds_dct_strong_public_bytes", "feds_fragment_dct_strong", "feds_defragment_dct_strong", "feds_fragment_dct_strong_batch",
+    "feds_defragment_dct_strong_batch", "feds_debug_strong_basis_host",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host", "feds_debug_launch_count",
 ]
 
@@ -62,6 +64,13 @@ def _load():
     lib.feds_fragment_dct_batch.argtypes = [vp, i, sz, i, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, C.c_uint, vp]
     lib.feds_defragment_dct_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, u8p, vp, vp, vp, sz, vp, vp, sz, C.c_uint, vp]
     lib.feds_fragment_dwt_batch.argtypes = lib.feds_fragment_dct_batch.argtypes
+    lib.feds_fragment_dct_strong.argtypes = lib.feds_fragment_dct.argtypes
+    lib.feds_defragment_dct_strong.argtypes = lib.feds_defragment_dct.argtypes
+    lib.feds_fragment_dct_strong_batch.argtypes = lib.feds_fragment_dct_batch.argtypes
+    lib.feds_defragment_dct_strong_batch.argtypes = lib.feds_defragment_dct_batch.argtypes
+    lib.feds_dct_strong_public_bytes.restype = sz
+    lib.feds_dct_strong_public_bytes.argtypes = [i, i, i]
+    lib.feds_debug_strong_basis_host.argtypes = [vp]
     lib.feds_defragment_dwt_batch.argtypes = lib.feds_defragment_dct_batch.argtypes
     lib.feds_fragment_dct_host_scratch_bytes.restype = sz
     lib.feds_fragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
@@ -86,7 +95,8 @@ def _load():
     lib.feds_debug_launch_count.argtypes = []
     for name in ["feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
                  "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
-                 "feds_fragment_dct_host", "feds_defragment_dct_host",
+                 "feds_fragment_dct_host", "feds_defragment_dct_host", "feds_fragment_dct_strong", "feds_defragment_dct_strong",
+                 "feds_fragment_dct_strong_batch", "feds_defragment_dct_strong_batch",
                  "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt"]:
         getattr(lib, name).restype = i
     return lib
@@ -195,6 +205,31 @@ def defragment_dct(priv, pub, w, h, c, k, key, nonce, expected=None, stream=None
     return out, flags
 
 
+def fragment_dct_strong(image, k, key, nonce, stream=None, workspace=None):
+    """feds_fragment_dct_strong: image -> (private ciphertext, public uint8[w*h*c], digests[64]) at the strong level"""
+    image, w, h, c = _hwc(image)
+    dev = image.device
+    priv = _u8(dct_private_bytes(w, h, c, k), dev)
+    pub = _u8(lib.feds_dct_strong_public_bytes(w, h, c), dev)
+    dg = _u8(64, dev)
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _on_stream(stream, priv, pub, dg, ws)
+    _check(lib.feds_fragment_dct_strong(_ptr(image), w, h, c, k, _k16(key), _k16(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws),
+                                        ws.numel(), _stream(stream)), "feds_fragment_dct_strong")
+    return priv[:dct_private_bytes(w, h, c, k)], pub[:w * h * c], dg
+
+
+def defragment_dct_strong(priv, pub, w, h, c, k, key, nonce, expected=None, stream=None, workspace=None):
+    dev = priv.device
+    out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
+    flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
+    ws = workspace if workspace is not None else _u8(workspace_bytes(w, h, c, k), dev)
+    _on_stream(stream, out, flags, ws)
+    _check(lib.feds_defragment_dct_strong(_ptr(priv), _ptr(pub), w, h, c, k, _k16(key), _k16(nonce), _ptr(expected), _ptr(out),
+                                          _ptr(flags), _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dct_strong")
+    return out, flags
+
+
 def verify_dct(priv, pub, w, h, c, k, expected, stream=None, workspace=None):
     """feds_verify_dct: integrity of the two fragments against their 64-byte digest pair, no key needed -> flags tensor [1]."""
     dev = priv.device
@@ -298,6 +333,36 @@ class DctBatch:
                                          self.k, _ptr(expected), _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), _stream(stream)),
                "feds_verify_dct_batch")
         return self.flags_out
+
+
+class StrongBatch:
+    """Pre-allocated buffers for feds_fragment_dct_strong_batch / feds_defragment_dct_strong_batch on n images of one shape."""
+
+    def __init__(self, n, w, h, c, k, device="cuda"):
+        self.n, self.w, self.h, self.c, self.k = n, w, h, c, k
+        self.image_bytes = w * h * c
+        self.priv_bytes = dct_private_bytes(w, h, c, k)
+        self.pub_bytes = w * h * c
+        self.priv_stride = (self.priv_bytes + 15) // 16 * 16
+        self.pub_stride = (self.pub_bytes + 15) // 16 * 16
+        self.priv = _u8(n * self.priv_stride, device)
+        self.pub = _u8(n * self.pub_stride, device)
+        self.digests = _u8(n * 64, device)
+        self.ws = _u8(n * workspace_bytes(w, h, c, k), device)
+        self.flags_out = torch.zeros(n, dtype=torch.int32, device=device)
+
+    def fragment(self, images, key, d_nonces, flags=FLAG_NONE, stream=None):
+        assert images.is_cuda and images.dtype == torch.uint8 and images.is_contiguous() and images.numel() == self.n * self.image_bytes
+        _check(lib.feds_fragment_dct_strong_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, self.k, _k16(key),
+                                                  _ptr(d_nonces), _ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride,
+                                                  _ptr(self.digests), _ptr(self.ws), self.ws.numel(), flags, _stream(stream)),
+               "feds_fragment_dct_strong_batch")
+
+    def defragment(self, images_out, key, d_nonces, expected=None, flags=FLAG_NONE, stream=None):
+        _check(lib.feds_defragment_dct_strong_batch(_ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, self.n, self.w,
+                                                    self.h, self.c, self.k, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
+                                                    self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
+                                                    _stream(stream)), "feds_defragment_dct_strong_batch")
 
 
 class DwtBatch:

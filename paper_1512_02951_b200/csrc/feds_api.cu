@@ -95,13 +95,14 @@ feds_status check_dct_args(int n_images, int w, int h, int c, int k) {
 }
 
 void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, const uint8_t key[16], const uint8_t *d_nonces,
-                     const uint8_t *nonce_host, bool digest) {
+                     const uint8_t *nonce_host, bool digest, bool strong = false) {
     memset(&p, 0, sizeof p);
     p.n_images = n_images; p.w = w; p.h = h; p.k = k;
     p.nbr = h / 8; p.nbc = w / 8; p.nlr = (p.nbc + G_BLOCKS - 1) / G_BLOCKS;
     p.leaves_per_image = (unsigned)c * p.nbr * p.nlr;
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
     p.one = 1u;
+    p.pub_words = strong ? 16 : 63 - k;
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
@@ -122,13 +123,13 @@ Route pick_route(const DctParams &p, int c, unsigned flags) {
 feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
                               const uint8_t key[16], const uint8_t *d_nonces, const uint8_t *nonce_host, uint8_t *d_private,
                               size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests,
-                              void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
+                              void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream, bool strong = false) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (flags & ~DCT_FLAGS) return FEDS_ERR_BAD_PARAM;
+    if (flags & ~(strong ? FEDS_FLAG_NO_DIGEST : DCT_FLAGS)) return FEDS_ERR_BAD_PARAM;
     if ((flags & FEDS_FLAG_FORCE_FUSED) && (flags & FEDS_FLAG_FORCE_SPLIT)) return FEDS_ERR_BAD_PARAM;
     const bool digest = !(flags & FEDS_FLAG_NO_DIGEST);
-    const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
+    const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = strong ? feds_dct_strong_public_bytes(w, h, c) : feds_dct_public_bytes(w, h, c, k);
     if (!d_images || !key || !d_private || (!d_public && pub_b) || (digest && (!d_digests || !d_workspace)) || (!d_nonces && !nonce_host))
         return FEDS_ERR_NULL_POINTER;
     if (image_stride < (size_t)w * h * c || private_stride < priv_b || public_stride < pub_b) return FEDS_ERR_BAD_PARAM;
@@ -139,13 +140,23 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
     if (digest && workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
 
     DctParams p;
-    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, digest);
+    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, digest, strong);
     p.generic_tiles = (flags & FEDS_FLAG_GENERIC_TILES) ? 1 : 0;
     p.images = d_images; p.image_stride = image_stride;
     p.priv = d_private; p.priv_stride = private_stride;
     p.pub = d_public; p.pub_stride = public_stride;
     uint8_t *ws = static_cast<uint8_t *>(d_workspace);
     p.leaves = (pl.nl > 1) ? ws : d_digests;  // a one-leaf fragment's root is its leaf digest
+    const bool pub_empty = !strong && k == 63;
+    if (strong) {   // PAPER.md 6.3.2: Part 1 under AES, the remainder pixels under a SHA-512 keystream; then the same Merkle digests
+        st = launch_fragment_strong(p, c, stream, !digest);
+        if (st != FEDS_OK) return st;
+        if (!digest) return FEDS_OK;
+        st = launch_leaves_hash(p, c, stream, true);
+        if (st != FEDS_OK) return st;
+        if (pl.nl > 1) return run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, d_digests, 32, 0, stream);
+        return FEDS_OK;
+    }
     if (digest) {
         const Route route = pick_route(p, c, flags);
         if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;
@@ -158,10 +169,10 @@ feds_status fragment_dct_impl(const uint8_t *d_images, int n_images, size_t imag
         }
         if (st != FEDS_OK) return st;
         if (pl.nl > 1) {
-            st = run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, d_digests, 32, k == 63 ? 1 : 0, stream);
+            st = run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, d_digests, 32, pub_empty ? 1 : 0, stream);
             if (st != FEDS_OK) return st;
         }
-        if (k == 63) {
+        if (pub_empty) {
             st = launch_empty_public_roots(d_digests, n_images, stream);
             if (st != FEDS_OK) return st;
         }
@@ -178,7 +189,7 @@ uint8_t *verification_leaves(const DctPlan &pl, int n_images, uint8_t *ws) { ret
 // leaf digests (already enqueued) -> roots -> flags[n] = bit0 private mismatch | bit1 public mismatch
 feds_status finish_verification(const DctParams &p, const DctPlan &pl, int n_images, int k, uint8_t *ws, const uint8_t *d_expected,
                                 uint32_t *d_flags, cudaStream_t stream) {
-    (void)p;
+    if (p.pub_words != 0) k = 0;   // only an EMPTY public fragment (first level, k = 63) takes the SHA-256("") root
     uint8_t *roots = verification_roots(pl, n_images, ws);
     if (pl.nl > 1) {
         const feds_status st = run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, roots, 32, k == 63 ? 1 : 0, stream);
@@ -194,13 +205,13 @@ feds_status finish_verification(const DctParams &p, const DctPlan &pl, int n_ima
 feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
                                 int n_images, int w, int h, int c, int k, const uint8_t key[16], const uint8_t *d_nonces,
                                 const uint8_t *nonce_host, const uint8_t *d_expected, uint8_t *d_images_out, size_t image_stride,
-                                uint32_t *d_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
+                                uint32_t *d_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream, bool strong = false) {
     feds_status st = check_dct_args(n_images, w, h, c, k);
     if (st != FEDS_OK) return st;
-    if (flags & ~DCT_FLAGS) return FEDS_ERR_BAD_PARAM;
+    if (flags & ~(strong ? FEDS_FLAG_NO_DIGEST : DCT_FLAGS)) return FEDS_ERR_BAD_PARAM;
     if ((flags & FEDS_FLAG_FORCE_FUSED) && (flags & FEDS_FLAG_FORCE_SPLIT)) return FEDS_ERR_BAD_PARAM;
     const bool verify = d_expected != nullptr && !(flags & FEDS_FLAG_NO_DIGEST);
-    const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = feds_dct_public_bytes(w, h, c, k);
+    const size_t priv_b = feds_dct_private_bytes(w, h, c, k), pub_b = strong ? feds_dct_strong_public_bytes(w, h, c) : feds_dct_public_bytes(w, h, c, k);
     if (!d_private || (!d_public && pub_b) || !key || !d_images_out || (!d_nonces && !nonce_host) || (verify && (!d_flags || !d_workspace)))
         return FEDS_ERR_NULL_POINTER;
     if (image_stride < (size_t)w * h * c || private_stride < priv_b || public_stride < pub_b) return FEDS_ERR_BAD_PARAM;
@@ -211,11 +222,21 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
     if (verify && workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
 
     DctParams p;
-    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, verify);
+    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, verify, strong);
     p.generic_tiles = (flags & FEDS_FLAG_GENERIC_TILES) ? 1 : 0;
     p.images_out = d_images_out; p.image_stride = image_stride;
     p.priv = const_cast<uint8_t *>(d_private); p.priv_stride = private_stride;
     p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
+    if (strong) {
+        if (verify) {
+            p.leaves = verification_leaves(pl, n_images, static_cast<uint8_t *>(d_workspace));
+            st = launch_leaves_hash(p, c, stream, true);
+            if (st != FEDS_OK) return st;
+        }
+        st = launch_defragment_strong(p, c, stream, !verify);
+        if (st != FEDS_OK) return st;
+        return verify ? finish_verification(p, pl, n_images, k, static_cast<uint8_t *>(d_workspace), d_expected, d_flags, stream) : FEDS_OK;
+    }
     if (verify) {
         p.leaves = verification_leaves(pl, n_images, static_cast<uint8_t *>(d_workspace));
         // Verification and reconstruction read the same fragments. Fused route: one warp-specialised kernel whose hash warps
@@ -527,6 +548,51 @@ feds_status feds_verify_dct_batch(const uint8_t *d_private, size_t private_strid
                            d_workspace, workspace_bytes, stream);
 }
 
+// ------------------------------------------------------------------------------------------------ strong level
+size_t feds_dct_strong_public_bytes(int w, int h, int c) {
+    if (!dct_dims_ok(w, h) || !chan_ok(c)) return 0;
+    return (size_t)w * h * c;
+}
+
+feds_status feds_fragment_dct_strong(const uint8_t *d_image, int w, int h, int c, int k, const uint8_t key[16], const uint8_t nonce[16],
+                                     uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
+                                     feds_stream_t stream) {
+    if (!nonce) return FEDS_ERR_NULL_POINTER;
+    return fragment_dct_impl(d_image, 1, (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), w, h, c, k, key, nullptr, nonce,
+                             d_private, feds_dct_private_bytes(w, h, c, k), d_public, feds_dct_strong_public_bytes(w, h, c), d_digests,
+                             d_workspace, workspace_bytes, FEDS_FLAG_NONE, stream, true);
+}
+
+feds_status feds_fragment_dct_strong_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
+                                           const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private, size_t private_stride,
+                                           uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                                           size_t workspace_bytes, unsigned flags, feds_stream_t stream) {
+    if (!d_nonces) return FEDS_ERR_NULL_POINTER;
+    return fragment_dct_impl(d_images, n_images, image_stride, w, h, c, k, key, d_nonces, nullptr, d_private, private_stride, d_public,
+                             public_stride, d_digests, d_workspace, workspace_bytes, flags, stream, true);
+}
+
+feds_status feds_defragment_dct_strong(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k, const uint8_t key[16],
+                                       const uint8_t nonce[16], const uint8_t *d_expected_digests, uint8_t *d_image_out,
+                                       uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, feds_stream_t stream) {
+    if (!nonce) return FEDS_ERR_NULL_POINTER;
+    return defragment_dct_impl(d_private, feds_dct_private_bytes(w, h, c, k), d_public, feds_dct_strong_public_bytes(w, h, c), 1, w, h, c, k,
+                               key, nullptr, nonce, d_expected_digests, d_image_out,
+                               (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), d_verify_flags, d_workspace, workspace_bytes,
+                               FEDS_FLAG_NONE, stream, true);
+}
+
+feds_status feds_defragment_dct_strong_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                             int n_images, int w, int h, int c, int k, const uint8_t key[16], const uint8_t *d_nonces,
+                                             const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                             uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                             feds_stream_t stream) {
+    if (!d_nonces) return FEDS_ERR_NULL_POINTER;
+    return defragment_dct_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, k, key, d_nonces, nullptr,
+                               d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, flags,
+                               stream, true);
+}
+
 // ------------------------------------------------------------------------------------------------ DWT
 feds_status feds_fragment_dwt(const uint8_t *d_image, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t nonce[16],
                               uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
@@ -766,6 +832,8 @@ void feds_debug_dct8x8_host(const float in[64], float out[64], int inverse) {
     if (inverse) idct8x8(v); else dct8x8(v);
     memcpy(out, v, sizeof v);
 }
+
+void feds_debug_strong_basis_host(int32_t out[64 * 64]) { strong_basis_host(out); }
 
 void feds_debug_zigzag_host(int out[64]) {
     for (int z = 0; z < 64; ++z) out[z] = h_zigzag.pos[z];

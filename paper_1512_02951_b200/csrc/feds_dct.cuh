@@ -28,6 +28,7 @@ struct DctParams {
     unsigned leaves_per_image;  // C * nbr * nlr
     unsigned long long total_leaves;
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
+    int pub_words;      // 32-bit words per block in the public fragment: 63 - k (first level) or 16 (strong level: 64 pixel bytes)
     int generic_tiles;  // 1: digest-free path on the generic tile kernels even where the bulk-copy kernels apply (FEDS_FLAG_GENERIC_TILES)
 };
 

@@ -56,6 +56,10 @@ feds_status launch_defragment_tma(const DctParams &p, int c, cudaStream_t stream
 feds_status launch_fragment_tile(const DctParams &p, int c, cudaStream_t stream, bool profile);
 feds_status launch_defragment_tile(const DctParams &p, int c, cudaStream_t stream, bool profile);
 feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream, bool profile);
+// ---- feds_k_dct_strong.cu: the report's strong level of protection (one thread per block; any image size)
+feds_status launch_fragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile);
+feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile);
+void strong_basis_host(int32_t out[64 * 64]);
 // ---- feds_k_hash.cu: Merkle upper levels, stream leaves, AES-CTR stream, digest compare
 feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
                      int skip_odd, cudaStream_t stream);

@@ -1,0 +1,40 @@
+// feds_k_dct_strong.cu — launchers of the strong-level kernels (feds_dct_strong.cuh; PAPER.md 6.3.2).
+#include "feds_dct_strong.cuh"
+#include "feds_host.h"
+
+namespace feds {
+
+namespace {
+constexpr size_t STRONG_SMEM = (size_t)(AES_TABLE_WORDS + 64 * STRONG_THREADS) * 4;
+constexpr StrongBasis h_strong_basis = make_strong_basis();
+}  // namespace
+
+void strong_basis_host(int32_t out[64 * 64]) {
+    for (int i = 0; i < 64 * 64; ++i) out[i] = h_strong_basis.B[i];
+}
+
+feds_status launch_fragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile) {
+    const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nbc;
+    const unsigned grid = (unsigned)((threads + STRONG_THREADS - 1) / STRONG_THREADS);
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (c == 1) fragment_dct_strong_kernel<1><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    else if (c == 3) fragment_dct_strong_kernel<3><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    else fragment_dct_strong_kernel<4><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
+feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile) {
+    const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nbc;
+    const unsigned grid = (unsigned)((threads + STRONG_THREADS - 1) / STRONG_THREADS);
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (c == 1) defragment_dct_strong_kernel<1><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    else if (c == 3) defragment_dct_strong_kernel<3><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    else defragment_dct_strong_kernel<4><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
+}  // namespace feds

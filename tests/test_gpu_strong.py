@@ -1,0 +1,122 @@
+"""GPU parity of the strong level of protection (feds_fragment_dct_strong / feds_defragment_dct_strong; PAPER.md 6.3.2, P:502-516;
+DESIGN.md 2.3) through the C ABI against the oracle (oracle/feds_oracle_strong.c).
+
+Part 1 is float32 DCT output, so more than one result is correct (any coefficient within 1e-3) and -- a hash seeing every bit -- the
+keystream legitimately differs between two correct DCTs. Parity is the two-stage protocol of DESIGN.md section 3:
+  (i)   the GPU's Part 1, decrypted with the oracle's AES-CTR, against the oracle's double DCT: max abs error <= 1e-3;
+  (ii)  the oracle fed the GPU's own Part 1 coefficients: ciphertext, all public bytes (fixed-point remainder and SHA-512 keystream)
+        and both Merkle digests bit-exact;
+  (iii) exact uint8 round trips: GPU(GPU), oracle(GPU), GPU(oracle) -- exact by construction (S1), also across implementations.
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def b():
+    from paper_1512_02951_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def check(orc, b, img, k, seed):
+    h, w, c = img.shape
+    key, nonce = synth.key_nonce(seed)
+    d_img = torch.from_numpy(img).cuda()
+    priv, pub, dg = b.fragment_dct_strong(d_img, k, key, nonce)
+    torch.cuda.synchronize()
+    pv, pb, dgb = priv.cpu().numpy(), pub.cpu().numpy(), dg.cpu().numpy().tobytes()
+    nb, P = c * (h // 8) * (w // 8), k + 1
+    assert pv.size == 4 * nb * P and pb.size == w * h * c
+    part1 = np.frombuffer(orc.aes128_ctr_xor(key, nonce, pv.tobytes()), dtype="<f4").reshape(nb, P)
+    ref = orc.dct_coefficients(img)[:, :P]
+    assert np.abs(part1.astype(np.float64) - ref).max() <= TOL                              # (i)
+    p2, q2, d2 = orc.fragment_strong_from_priv32(img, part1, k, key, nonce)                 # (ii)
+    assert (p2 == pv).all(), "private ciphertext differs"
+    assert (q2 == pb).all(), "public bytes differ"
+    assert d2 == dgb, "digests differ"
+    rec, flags = b.defragment_dct_strong(priv, pub, w, h, c, k, key, nonce, expected=dg)    # (iii)
+    torch.cuda.synchronize()
+    assert int(flags.item()) == 0 and torch.equal(rec, d_img)
+    rec2, _ = b.defragment_dct_strong(priv, pub, w, h, c, k, key, nonce)
+    assert torch.equal(rec2, d_img)
+    orec, ofl = orc.defragment_dct_strong(pv, pb, w, h, c, k, key, nonce, expected=dgb)
+    assert ofl == 0 and (orec == img).all()
+    op, oq, odg = orc.fragment_dct_strong(img, k, key, nonce)
+    rec3, fl3 = b.defragment_dct_strong(torch.from_numpy(op).cuda(), torch.from_numpy(oq).cuda(), w, h, c, k, key, nonce,
+                                        expected=torch.frombuffer(bytearray(odg), dtype=torch.uint8).cuda())
+    torch.cuda.synchronize()
+    assert int(fl3.item()) == 0 and torch.equal(rec3, d_img)
+    return d_img, priv, pub, dg, key, nonce
+
+
+@pytest.mark.parametrize("w,h,c,k", [(8, 8, 1, 0), (8, 8, 1, 5), (16, 16, 4, 63), (64, 8, 1, 3), (72, 24, 1, 5), (1080, 16, 3, 5), (136, 40, 4, 9),
+                                     (512, 512, 1, 5), (256, 264, 3, 5), (520, 24, 3, 26), (520, 24, 3, 27), (64, 64, 1, 32), (40, 8, 3, 4),
+                                     (1920, 136, 3, 5), (2056, 8, 1, 1)])
+def test_strong_parity_and_round_trips(orc, b, w, h, c, k):
+    check(orc, b, synth.image(w, h, c, seed=w + 3 * h + c + k, rectangles=2 if w >= 64 and h >= 16 else 0), k, seed=w * 5 + k)
+
+
+@pytest.mark.parametrize("kind", ["zeros", "ones", "checker", "random", "impulse"])
+@pytest.mark.parametrize("c", [1, 3, 4])
+def test_strong_special_images(orc, b, kind, c):
+    check(orc, b, synth.special(kind, 96, 32, c, seed=c), 5, seed=13)
+
+
+def test_strong_verify_flags_and_damage_confinement(orc, b):
+    """A flipped public bit is flagged and damages exactly one pixel; a flipped Part 1 bit is flagged and damages at most the
+    blocks whose AES counter block it shares (their low-pass image and their SHA-512 keystream change)."""
+    img = synth.image(256, 64, 3, seed=21, rectangles=2)
+    d_img, priv, pub, dg, key, nonce = check(orc, b, img, 5, seed=21)
+    q2 = pub.clone(); q2[1000] ^= 0x04
+    rec, fl = b.defragment_dct_strong(priv, q2, 256, 64, 3, 5, key, nonce, expected=dg)
+    assert int(fl.item()) == 2 and int((rec != d_img).sum().item()) == 1
+    p2 = priv.clone(); p2[24 * 7 + 2] ^= 0x40     # a byte of block 7's Part 1
+    rec, fl = b.defragment_dct_strong(p2, pub, 256, 64, 3, 5, key, nonce, expected=dg)
+    assert int(fl.item()) == 1
+    bad = (rec != d_img).any(dim=2).cpu().numpy()
+    assert bad.any() and not bad[8:, :].any() and not bad[:, 64:].any()      # confined to block 7 (row 0, columns 56..63)
+
+
+def test_strong_batch_equals_singles(orc, b):
+    n, w, h, c, k = 5, 264, 40, 3, 5
+    key, nonce = synth.key_nonce(31)
+    batch = b.StrongBatch(n, w, h, c, k)
+    nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
+    imgs = np.stack([synth.image(w, h, c, seed=300 + i, rectangles=1) for i in range(n)])
+    d_imgs, d_non = torch.from_numpy(imgs).cuda(), torch.from_numpy(nonces).cuda()
+    batch.fragment(d_imgs, key, d_non)
+    torch.cuda.synchronize()
+    for i in range(n):
+        priv, pub, dg = b.fragment_dct_strong(d_imgs[i].contiguous(), k, key, nonces[i].tobytes())
+        assert torch.equal(batch.priv[i * batch.priv_stride:i * batch.priv_stride + batch.priv_bytes], priv)
+        assert torch.equal(batch.pub[i * batch.pub_stride:i * batch.pub_stride + batch.pub_bytes], pub)
+        assert torch.equal(batch.digests[64 * i:64 * i + 64], dg)
+    out = torch.zeros_like(d_imgs)
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    batch.pub[2 * batch.pub_stride + 5] ^= 1
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    assert batch.flags_out.cpu().tolist() == [0, 0, 2, 0, 0]
+    # digest-free: same fragments, no digests written
+    plain = b.StrongBatch(n, w, h, c, k)
+    plain.digests.fill_(0xEE)
+    plain.fragment(d_imgs, key, d_non, flags=b.FLAG_NO_DIGEST)
+    batch.pub[2 * batch.pub_stride + 5] ^= 1
+    for i in range(n):   # (the bytes between an image's fragment and the next stride are not written)
+        assert torch.equal(plain.priv[i * plain.priv_stride:i * plain.priv_stride + plain.priv_bytes],
+                           batch.priv[i * batch.priv_stride:i * batch.priv_stride + batch.priv_bytes])
+        assert torch.equal(plain.pub[i * plain.pub_stride:i * plain.pub_stride + plain.pub_bytes],
+                           batch.pub[i * batch.pub_stride:i * batch.pub_stride + batch.pub_bytes])
+    assert int((plain.digests != 0xEE).sum().item()) == 0
+
+
+def test_strong_full_hd_image(orc, b):
+    """one 1920x1080 RGB image, k = 5 (the report's default selection): stage (ii) on the whole image, exact round trip"""
+    check(orc, b, synth.image(1920, 1080, 3, seed=8, rectangles=8), 5, seed=8)

@@ -138,3 +138,15 @@ def test_header_is_plain_c(tmp_path):
     res = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), str(src)],
                          capture_output=True, text=True)
     assert res.returncode == 0, res.stderr
+
+
+def test_strong_level_basis_table_equals_the_oracles():
+    """The strong level's fixed-point DCT basis B[z][p] = rne(4096 b_z(p)) decides stored bytes, so the library's
+    table (built at compile time from a Taylor series) and the oracle's (libm) must agree in all 4096 entries."""
+    import ctypes as C
+    import numpy as np
+    import oracle
+    from paper_1512_02951_b200 import binding
+    out = np.zeros(4096, dtype=np.int32)
+    binding.lib.feds_debug_strong_basis_host(out.ctypes.data)
+    assert (out.reshape(64, 64) == oracle.strong_basis()).all()
