@@ -449,7 +449,7 @@ def main():
         hashed_bytes = n * (w // 8) * (h // 8) * c * 256
         alg_bytes = hashed_bytes + n * nl * 64      # read every stored byte once, write 2 x 32 B of leaf digest per leaf
         achieved = alu_ops / (hash_ms * 1e-3) / 1e12
-        vname = "dct_leaves_hash_kernel<%d>" % c
+        vname = ("dct_leaves_hash_coop_kernel<%d>" if n * nl <= 592 else "dct_leaves_hash_kernel<%d>") % c   # few leaves: the latency form
         traffic, traffic_src = stored_traffic(vname, args.workload, n)
         ceiling = None
         peaks_bin = os.path.join(ROOT, "paper_1512_02951_b200", "feds_peaks")
@@ -508,6 +508,24 @@ def main():
             stages["fused_route_forced"] = {"fragment_ms": ff_ms, "defragment_verify_ms": fd_ms}
         except B.FedsError as e:
             stages["fused_route_forced"] = {"unsupported": str(e)}
+
+    if kind == "dct" and rank == 0:
+        # the report's strong level of protection on the same batch (Part 1 under AES, remainder pixels under a
+        # SHA-512 keystream per 8x8 block), with and without the Merkle digests
+        sb = B.StrongBatch(n, w, h, c, kl, device=dev)
+        s_non = torch.from_numpy(sharding.nonces_for(nonce, rank * n, n, priv_bytes=sb.priv_bytes)).to(dev)
+        sf = timed(lambda: sb.fragment(d_imgs, key, s_non), reps=3)
+        sd = timed(lambda: sb.defragment(d_out, key, s_non, expected=sb.digests), reps=3)
+        assert torch.equal(d_out, d_imgs) and int(sb.flags_out.abs().sum().item()) == 0
+        sf0 = timed(lambda: sb.fragment(d_imgs, key, s_non, flags=B.FLAG_NO_DIGEST), reps=3)
+        sd0 = timed(lambda: sb.defragment(d_out, key, s_non, flags=B.FLAG_NO_DIGEST), reps=3)
+        assert torch.equal(d_out, d_imgs)
+        n_blocks = n * c * (h // 8) * (w // 8)
+        stages["strong_level"] = {"fragment_ms": sf, "defragment_verify_ms": sd, "fragment_nodigest_ms": sf0, "defragment_nodigest_ms": sd0,
+                                  "fragment_nodigest_MBps": step_image_bytes / (sf0 * 1e-3) / 1e6,
+                                  "sha512_per_s": n_blocks / (sf0 * 1e-3),
+                                  "note": "one SHA-512 per 8x8 block (the report estimates 136 MH/s on its GTX 780, P:678)"}
+        del sb
 
     if kind == "dwt":
         # dominant kernel: stream_leaves_kernel (SHA-256 of every 2048-byte leaf of both fragments), ALU-bound like the DCT path
