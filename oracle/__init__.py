@@ -319,3 +319,73 @@ def strong_remainder(image, k) -> np.ndarray:
     rc = lib().orc_strong_remainder(pi, w, h, c, k, out.ctypes.data_as(C.POINTER(C.c_int16)))
     assert rc == 0, rc
     return out
+
+
+# ------------------------------------------------------------------------------------------ packed storage (feds_oracle_packed.c)
+def packed_private_bytes(w, h, c, k, ac_bits, g=G_BLOCKS):
+    lib().orc_packed_private_bytes.restype = C.c_uint64
+    return int(lib().orc_packed_private_bytes(w, h, c, k, ac_bits, g))
+
+
+def packed_quantise(cf, is_dc, ac_bits):
+    lib().orc_packed_quantise.argtypes = [C.c_float, C.c_int, C.c_int]
+    return int(lib().orc_packed_quantise(C.c_float(cf), int(is_dc), ac_bits))
+
+
+def pack_group(q, k, ac_bits) -> bytes:
+    """q: int32 [nblk][k+1] -> the bytes of one leaf group"""
+    q = np.ascontiguousarray(q, dtype=np.int32).reshape(-1, k + 1)
+    out = np.zeros((q.shape[0] * (11 + k * ac_bits) + 7) // 8 + 8, dtype=np.uint8)
+    lib().orc_pack_group.restype = C.c_uint64
+    n = lib().orc_pack_group(q.ctypes.data_as(C.POINTER(C.c_int32)), q.shape[0], k, ac_bits, out.ctypes.data_as(C.POINTER(C.c_uint8)))
+    return out[:n].tobytes()
+
+
+def unpack_group(data, nblk, k, ac_bits) -> np.ndarray:
+    a, p = _u8(np.frombuffer(bytes(data), dtype=np.uint8))
+    q = np.zeros((nblk, k + 1), dtype=np.int32)
+    lib().orc_unpack_group.restype = C.c_uint64
+    lib().orc_unpack_group(p, nblk, k, ac_bits, q.ctypes.data_as(C.POINTER(C.c_int32)))
+    return q
+
+
+def fragment_dct_packed(image, k, ac_bits, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    """image -> (private: packed integers under AES-CTR, public: remainder pixels uint8 [block][64], digests[64], q int32 [nb][k+1])"""
+    img, h, w, c = _img(image)
+    nb = (w // 8) * (h // 8) * c
+    priv = np.zeros(packed_private_bytes(w, h, c, k, ac_bits, g), dtype=np.uint8)
+    pub = np.zeros(w * h * c, dtype=np.uint8)
+    q = np.zeros((nb, k + 1), dtype=np.int32)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_dct_packed(img.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c, k, ac_bits, _key(key), _key(nonce), g, fanout,
+                                       priv.ctypes.data_as(C.POINTER(C.c_uint8)), pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg,
+                                       q.ctypes.data_as(C.POINTER(C.c_int32)))
+    assert rc == 0, rc
+    return priv, pub, bytes(dg), q
+
+
+def fragment_packed_from_q(image, q, k, ac_bits, key, nonce, g=G_BLOCKS, fanout=FANOUT):
+    """stage (ii): everything after the quantisation from given integers q[b][z <= k]"""
+    img, h, w, c = _img(image)
+    q = np.ascontiguousarray(q, dtype=np.int32)
+    assert q.size == (w // 8) * (h // 8) * c * (k + 1)
+    priv = np.zeros(packed_private_bytes(w, h, c, k, ac_bits, g), dtype=np.uint8)
+    pub = np.zeros(w * h * c, dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_packed_from_q(img.ctypes.data_as(C.POINTER(C.c_uint8)), q.ctypes.data_as(C.POINTER(C.c_int32)), w, h, c, k, ac_bits,
+                                          _key(key), _key(nonce), g, fanout, priv.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                          pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    assert rc == 0, rc
+    return priv, pub, bytes(dg)
+
+
+def defragment_dct_packed(priv, pub, w, h, c, k, ac_bits, key, nonce, expected=None, g=G_BLOCKS, fanout=FANOUT):
+    pa, pp = _u8(priv)
+    qa, qp = _u8(pub)
+    out = np.zeros((h, w, c), dtype=np.uint8)
+    fl = C.c_uint32(0)
+    exp = (C.c_uint8 * 64).from_buffer_copy(bytes(expected)) if expected is not None else None
+    rc = lib().orc_defragment_dct_packed(pp, qp, w, h, c, k, ac_bits, _key(key), _key(nonce), g, fanout, exp,
+                                         out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(fl))
+    assert rc == 0, rc
+    return out, int(fl.value)
