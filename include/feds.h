@@ -142,6 +142,39 @@ feds_status feds_defragment_dct_strong_batch(const uint8_t *d_private, size_t pr
                                              unsigned flags, feds_stream_t stream);
 
 /*
+ * Packed integer coefficient storage (PAPER.md 6.4.3, Table 5; byte format: DESIGN.md 2.4). Part 1 of every block is
+ * stored as integers: DC rounded into 11 bits ("DC coefficients are bounded by 2040"), every AC rounded into a sign-magnitude
+ * field of ac_bits = 11 or 8 bits, clamped to its range; the fields of the (up to) 8 blocks of a leaf group form one little-endian
+ * bit stream, so a full group takes exactly 11 + k*ac_bits bytes: 12.9 % (11-bit) or 9.96 % (8-bit) of a gray image at k = 5, as
+ * P:599 prints. The private fragment is that stream under AES-128-CTR; the public fragment is w*h*c bytes, uint8 [block][64]: the
+ * remainder pixels x - L modulo 256 ("IDCT of the rest"), taken against the quantised Part 1 in exact fixed-point arithmetic,
+ * so that the inverse reproduces every pixel exactly with either storage. Digests: Merkle roots of the stored bytes (private leaf =
+ * one group's bytes, public leaf = 8 blocks x 64 bytes).
+ *   workspace: feds_dct_packed_workspace_bytes() per image (digest levels + room for the decrypted private fragment).
+ *   errors as feds_fragment_dct; ac_bits other than 11 or 8: FEDS_ERR_BAD_PARAM. d_digests and the workspace are required.
+ */
+size_t feds_dct_packed_private_bytes(int w, int h, int c, int k, int ac_bits);
+size_t feds_dct_packed_workspace_bytes(int w, int h, int c, int k, int ac_bits);
+feds_status feds_fragment_dct_packed(const uint8_t *d_image, int w, int h, int c, int k, int ac_bits, const uint8_t key[16],
+                                     const uint8_t nonce[16], uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests,
+                                     void *d_workspace, size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_defragment_dct_packed(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k, int ac_bits,
+                                       const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                       uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
+                                       size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_fragment_dct_packed_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c,
+                                           int k, int ac_bits, const uint8_t key[16], const uint8_t *d_nonces,
+                                           uint8_t *d_private, size_t private_stride, uint8_t *d_public, size_t public_stride,
+                                           uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
+                                           feds_stream_t stream);
+feds_status feds_defragment_dct_packed_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public,
+                                             size_t public_stride, int n_images, int w, int h, int c, int k, int ac_bits,
+                                             const uint8_t key[16], const uint8_t *d_nonces,
+                                             const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                             uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                                             feds_stream_t stream);
+
+/*
  * feds_fragment_dwt / feds_defragment_dwt — rows D1-D8: level shift -128, `levels`-level whole-image
  * Le Gall 5/3 integer lifting, rows then columns, LL_levels -> private under AES-128-CTR,
  * the other subbands -> public (order: channel, level L..1, HL, LH, HH, row-major int16 LE), SHA-256 Merkle

@@ -103,6 +103,7 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
     p.one = 1u;
     p.pub_words = strong ? 16 : 63 - k;
+    p.priv_words = k + 1;
     (void)digest;
     p.d_nonces = d_nonces;
     if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
@@ -445,6 +446,96 @@ feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride,
     return FEDS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- packed integer storage
+bool packed_args_ok(int ac_bits) { return ac_bits == 11 || ac_bits == 8; }
+unsigned packed_bits_per_block(int k, int ac_bits) { return 11u + (unsigned)k * (unsigned)ac_bits; }
+size_t packed_row_bytes(int w, int k, int ac_bits) {
+    const unsigned nbc = (unsigned)(w / 8), b = packed_bits_per_block(k, ac_bits);
+    return (size_t)(nbc / G_BLOCKS) * b + ((nbc % G_BLOCKS) ? ((size_t)(nbc % G_BLOCKS) * b + 7) / 8 : 0);
+}
+void fill_packed_params(DctParams &p, int w, int k, int ac_bits) {
+    p.pub_words = 16;
+    p.priv_words = 0;   // the word-wise leaf-hash kernels skip the private fragment: packed_private_leaves_kernel hashes it
+    p.ac_bits = ac_bits;
+    p.packed_group_bytes = packed_bits_per_block(k, ac_bits);
+    p.packed_row_bytes = packed_row_bytes(w, k, ac_bits);
+}
+
+feds_status fragment_packed_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k, int ac_bits,
+                                 const uint8_t key[16], const uint8_t *nonce_host, const uint8_t *d_nonces, uint8_t *d_private,
+                                 size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                                 size_t workspace_bytes, cudaStream_t stream) {
+    feds_status st = check_dct_args(n_images, w, h, c, k);
+    if (st != FEDS_OK) return st;
+    if (!packed_args_ok(ac_bits)) return FEDS_ERR_BAD_PARAM;
+    const size_t priv_b = feds_dct_packed_private_bytes(w, h, c, k, ac_bits), pub_b = (size_t)w * h * c;
+    if (!d_images || !key || !d_private || !d_public || !d_digests || !d_workspace || (!d_nonces && !nonce_host)) return FEDS_ERR_NULL_POINTER;
+    if (image_stride < pub_b || private_stride < priv_b || public_stride < pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images) || misaligned(d_private) || misaligned(d_public) || misaligned(d_digests) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    const DctPlan pl = dct_plan(w, h, c);
+    if (workspace_bytes < feds_dct_packed_workspace_bytes(w, h, c, k, ac_bits) * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    DctParams p;
+    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, true);
+    fill_packed_params(p, w, k, ac_bits);
+    p.images = d_images; p.image_stride = image_stride;
+    p.priv = d_private; p.priv_stride = private_stride;
+    p.pub = d_public; p.pub_stride = public_stride;
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    p.leaves = (pl.nl > 1) ? ws : d_digests;
+    st = launch_fragment_packed(p, c, stream, false);
+    if (st != FEDS_OK) return st;
+    st = launch_aes_ctr(d_private, private_stride, d_private, private_stride, priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
+    if (st != FEDS_OK) return st;
+    st = launch_leaves_hash(p, c, stream, true);       // public leaves (16 words per block)
+    if (st != FEDS_OK) return st;
+    st = launch_packed_private_leaves(p, c, stream);   // private leaves (the groups' bytes, as stored: ciphertext)
+    if (st != FEDS_OK) return st;
+    if (pl.nl > 1) return run_tree(ws, pl.nl, 2u * n_images, ws + pl.level0_bytes * n_images, d_digests, 32, 0, stream);
+    return FEDS_OK;
+}
+
+feds_status defragment_packed_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                   int n_images, int w, int h, int c, int k, int ac_bits, const uint8_t key[16], const uint8_t *nonce_host,
+                                   const uint8_t *d_nonces, const uint8_t *d_expected, uint8_t *d_images_out, size_t image_stride,
+                                   uint32_t *d_flags, void *d_workspace, size_t workspace_bytes, cudaStream_t stream) {
+    feds_status st = check_dct_args(n_images, w, h, c, k);
+    if (st != FEDS_OK) return st;
+    if (!packed_args_ok(ac_bits)) return FEDS_ERR_BAD_PARAM;
+    const size_t priv_b = feds_dct_packed_private_bytes(w, h, c, k, ac_bits), pub_b = (size_t)w * h * c;
+    if (!d_private || !d_public || !key || !d_images_out || !d_workspace || (!d_nonces && !nonce_host) || (d_expected && !d_flags))
+        return FEDS_ERR_NULL_POINTER;
+    if (image_stride < pub_b || private_stride < priv_b || public_stride < pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images_out) || misaligned(d_private) || misaligned(d_public) || misaligned(d_expected) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    const DctPlan pl = dct_plan(w, h, c);
+    if (workspace_bytes < feds_dct_packed_workspace_bytes(w, h, c, k, ac_bits) * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    DctParams p;
+    fill_dct_params(p, n_images, w, h, c, k, key, d_nonces, nonce_host, d_expected != nullptr);
+    fill_packed_params(p, w, k, ac_bits);
+    p.images_out = d_images_out; p.image_stride = image_stride;
+    p.priv = const_cast<uint8_t *>(d_private); p.priv_stride = private_stride;
+    p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
+    uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+    if (d_expected) {
+        p.leaves = verification_leaves(pl, n_images, ws);
+        st = launch_leaves_hash(p, c, stream, true);
+        if (st != FEDS_OK) return st;
+        st = launch_packed_private_leaves(p, c, stream);
+        if (st != FEDS_OK) return st;
+        st = finish_verification(p, pl, n_images, k, ws, d_expected, d_flags, stream);
+        if (st != FEDS_OK) return st;
+    }
+    // the decrypted private fragments live behind the digest workspace of the whole batch
+    const size_t plain_stride = round_up(priv_b, 256);
+    uint8_t *plain = ws + pl.per_image * (size_t)n_images;
+    st = launch_aes_ctr(d_private, private_stride, plain, plain_stride, priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
+    if (st != FEDS_OK) return st;
+    return launch_defragment_packed(p, c, plain, plain_stride, stream, d_expected == nullptr);
+}
+
 }  // namespace
 
 // =================================================================================================== C ABI
@@ -591,6 +682,51 @@ feds_status feds_defragment_dct_strong_batch(const uint8_t *d_private, size_t pr
     return defragment_dct_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, k, key, d_nonces, nullptr,
                                d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, flags,
                                stream, true);
+}
+
+// ------------------------------------------------------------------------------------------------ packed storage
+size_t feds_dct_packed_private_bytes(int w, int h, int c, int k, int ac_bits) {
+    if (!dct_dims_ok(w, h) || !chan_ok(c) || k < 0 || k > 63 || !packed_args_ok(ac_bits)) return 0;
+    return (size_t)c * (h / 8) * packed_row_bytes(w, k, ac_bits);
+}
+size_t feds_dct_packed_workspace_bytes(int w, int h, int c, int k, int ac_bits) {
+    const size_t pb = feds_dct_packed_private_bytes(w, h, c, k, ac_bits);
+    if (pb == 0) return 0;
+    return dct_plan(w, h, c).per_image + round_up(pb, 256);
+}
+feds_status feds_fragment_dct_packed(const uint8_t *d_image, int w, int h, int c, int k, int ac_bits, const uint8_t key[16],
+                                     const uint8_t nonce[16], uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests,
+                                     void *d_workspace, size_t workspace_bytes, feds_stream_t stream) {
+    if (!nonce) return FEDS_ERR_NULL_POINTER;
+    return fragment_packed_impl(d_image, 1, (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), w, h, c, k, ac_bits, key, nonce, nullptr,
+                                d_private, feds_dct_packed_private_bytes(w, h, c, k, ac_bits), d_public,
+                                (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), d_digests, d_workspace, workspace_bytes, stream);
+}
+feds_status feds_fragment_dct_packed_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, int k,
+                                           int ac_bits, const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private,
+                                           size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests,
+                                           void *d_workspace, size_t workspace_bytes, feds_stream_t stream) {
+    if (!d_nonces) return FEDS_ERR_NULL_POINTER;
+    return fragment_packed_impl(d_images, n_images, image_stride, w, h, c, k, ac_bits, key, nullptr, d_nonces, d_private, private_stride,
+                                d_public, public_stride, d_digests, d_workspace, workspace_bytes, stream);
+}
+feds_status feds_defragment_dct_packed(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int k, int ac_bits,
+                                       const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                       uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                                       feds_stream_t stream) {
+    if (!nonce) return FEDS_ERR_NULL_POINTER;
+    const size_t img_b = (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0);
+    return defragment_packed_impl(d_private, feds_dct_packed_private_bytes(w, h, c, k, ac_bits), d_public, img_b, 1, w, h, c, k, ac_bits, key,
+                                  nonce, nullptr, d_expected_digests, d_image_out, img_b, d_verify_flags, d_workspace, workspace_bytes, stream);
+}
+feds_status feds_defragment_dct_packed_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                             int n_images, int w, int h, int c, int k, int ac_bits, const uint8_t key[16],
+                                             const uint8_t *d_nonces, const uint8_t *d_expected_digests, uint8_t *d_images_out,
+                                             size_t image_stride, uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes,
+                                             feds_stream_t stream) {
+    if (!d_nonces) return FEDS_ERR_NULL_POINTER;
+    return defragment_packed_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, k, ac_bits, key, nullptr, d_nonces,
+                                  d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ DWT

@@ -29,6 +29,11 @@ struct DctParams {
     unsigned long long total_leaves;
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
     int pub_words;      // 32-bit words per block in the public fragment: 63 - k (first level) or 16 (strong level: 64 pixel bytes)
+    int priv_words;     // 32-bit words per block in the private fragment for the leaf-hash kernels: k + 1, or 0 = skip (packed storage)
+    // packed integer storage (feds_dct_packed.cuh)
+    int ac_bits;                  // 11 or 8
+    unsigned packed_group_bytes;  // 11 + k * ac_bits: bits per block = bytes per full group of 8 blocks
+    size_t packed_row_bytes;      // private bytes per block row of one channel
     int generic_tiles;  // 1: digest-free path on the generic tile kernels even where the bulk-copy kernels apply (FEDS_FLAG_GENERIC_TILES)
 };
 

@@ -306,7 +306,7 @@ __global__ void __launch_bounds__(LEAFHASH_THREADS) dct_leaves_hash_kernel(const
     if (gid >= 2 * p.total_leaves) return;
     const bool priv = gid >= p.total_leaves;
     const LeafCoord L = decode_leaf<C>(p, priv ? gid - p.total_leaves : gid);
-    const int W = priv ? p.k + 1 : p.pub_words;   // words per block in this fragment
+    const int W = priv ? p.priv_words : p.pub_words;   // words per block in this fragment
     if (W == 0) return;                           // k = 63 at the first level: the public fragment is empty, its root is written elsewhere
     const uint32_t *src = reinterpret_cast<const uint32_t *>(priv ? p.priv + (size_t)L.n * p.priv_stride : p.pub + (size_t)L.n * p.pub_stride) +
                           (size_t)L.b0 * W;
@@ -367,7 +367,7 @@ __global__ void __launch_bounds__(COOP_WARPS * 32) dct_leaves_hash_coop_kernel(c
     extern __shared__ __align__(16) uint32_t coop_smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const unsigned long long wid = (unsigned long long)blockIdx.x * COOP_WARPS + warp;
-    const int P = p.k + 1, Q = p.pub_words;
+    const int P = p.priv_words, Q = p.pub_words;
     if (wid < p.total_leaves) {   // a public leaf, by the whole warp
         if (Q == 0) return;
         const LeafCoord L = decode_leaf<C>(p, wid);
@@ -379,7 +379,7 @@ __global__ void __launch_bounds__(COOP_WARPS * 32) dct_leaves_hash_coop_kernel(c
     }
     // 32 private leaves, one per lane
     const unsigned long long gid = (wid - p.total_leaves) * 32 + lane;
-    if (gid >= p.total_leaves) return;
+    if (gid >= p.total_leaves || P == 0) return;
     const LeafCoord L = decode_leaf<C>(p, gid);
     const uint32_t *src = reinterpret_cast<const uint32_t *>(p.priv + (size_t)L.n * p.priv_stride) + (size_t)L.b0 * P;
     const unsigned nwords = (unsigned)(L.nblk * P), nblocks = (nwords * 4u + 9u + 63u) / 64u;

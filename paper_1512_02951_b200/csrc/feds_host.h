@@ -60,6 +60,10 @@ feds_status launch_leaves_hash(const DctParams &p, int c, cudaStream_t stream, b
 feds_status launch_fragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile);
 feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t stream, bool profile);
 void strong_basis_host(int32_t out[64 * 64]);
+// packed integer storage (same translation unit): one thread per (leaf group, channel); `plain` = decrypted private fragments
+feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t stream, bool profile);
+feds_status launch_defragment_packed(const DctParams &p, int c, const uint8_t *plain, size_t plain_stride, cudaStream_t stream, bool profile);
+feds_status launch_packed_private_leaves(const DctParams &p, int c, cudaStream_t stream);
 // ---- feds_k_hash.cu: Merkle upper levels, stream leaves, AES-CTR stream, digest compare
 feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
                      int skip_odd, cudaStream_t stream);

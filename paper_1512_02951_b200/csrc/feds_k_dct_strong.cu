@@ -1,5 +1,6 @@
-// feds_k_dct_strong.cu — launchers of the strong-level kernels (feds_dct_strong.cuh; PAPER.md 6.3.2).
-#include "feds_dct_strong.cuh"
+// feds_k_dct_strong.cu — launchers of the strong-level kernels (feds_dct_strong.cuh; PAPER.md 6.3.2) and of the packed-storage kernels
+// (feds_dct_packed.cuh; PAPER.md 6.4.3), which share the fixed-point basis table.
+#include "feds_dct_packed.cuh"
 #include "feds_host.h"
 
 namespace feds {
@@ -33,6 +34,38 @@ feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t str
     else if (c == 3) defragment_dct_strong_kernel<3><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
     else defragment_dct_strong_kernel<4><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p);
     if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
+// ---- packed integer storage: one thread per (leaf group, channel)
+feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t stream, bool profile) {
+    const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nlr;
+    const unsigned grid = (unsigned)((threads + PACKED_THREADS - 1) / PACKED_THREADS);
+    const size_t smem = (size_t)64 * PACKED_THREADS * 4;
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (c == 1) fragment_dct_packed_kernel<1><<<grid, PACKED_THREADS, smem, stream>>>(p);
+    else if (c == 3) fragment_dct_packed_kernel<3><<<grid, PACKED_THREADS, smem, stream>>>(p);
+    else fragment_dct_packed_kernel<4><<<grid, PACKED_THREADS, smem, stream>>>(p);
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+feds_status launch_defragment_packed(const DctParams &p, int c, const uint8_t *plain, size_t plain_stride, cudaStream_t stream, bool profile) {
+    const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nlr;
+    const unsigned grid = (unsigned)((threads + PACKED_THREADS - 1) / PACKED_THREADS);
+    const size_t smem = (size_t)64 * PACKED_THREADS * 4;
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    if (c == 1) defragment_dct_packed_kernel<1><<<grid, PACKED_THREADS, smem, stream>>>(p, plain, plain_stride);
+    else if (c == 3) defragment_dct_packed_kernel<3><<<grid, PACKED_THREADS, smem, stream>>>(p, plain, plain_stride);
+    else defragment_dct_packed_kernel<4><<<grid, PACKED_THREADS, smem, stream>>>(p, plain, plain_stride);
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+feds_status launch_packed_private_leaves(const DctParams &p, int c, cudaStream_t stream) {
+    const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nlr;
+    packed_private_leaves_kernel<<<(unsigned)((threads + PACKED_THREADS - 1) / PACKED_THREADS), PACKED_THREADS, 0, stream>>>(p, c);
     FEDS_LAUNCH_CHECK();
     return FEDS_OK;
 }
