@@ -526,6 +526,17 @@ def main():
                                   "sha512_per_s": n_blocks / (sf0 * 1e-3),
                                   "note": "one SHA-512 per 8x8 block (the report estimates 136 MH/s on its GTX 780, P:678)"}
         del sb
+        # the report's packed 11-bit storage: Part 1 as bit-packed integers, remainder pixels public
+        pk = B.PackedBatch(n, w, h, c, kl, 11, device=dev)
+        p_non = torch.from_numpy(sharding.nonces_for(nonce, rank * n, n, priv_bytes=pk.priv_bytes)).to(dev)
+        pf = timed(lambda: pk.fragment(d_imgs, key, p_non), reps=3)
+        pd = timed(lambda: pk.defragment(d_out, key, p_non, expected=pk.digests), reps=3)
+        assert torch.equal(d_out, d_imgs) and int(pk.flags_out.abs().sum().item()) == 0
+        stages["packed_11bit_storage"] = {"fragment_ms": pf, "defragment_verify_ms": pd, "fragment_MBps": step_image_bytes / (pf * 1e-3) / 1e6,
+                                          "private_fraction_of_image": pk.priv_bytes / float(img_bytes),
+                                          "stored_bytes_per_pixel": (pk.priv_bytes + pk.pub_bytes) / float(img_bytes),
+                                          "note": "the digests cover stored_bytes_per_pixel bytes per pixel-channel instead of 4 (float32 storage)"}
+        del pk
 
     if kind == "dwt":
         # dominant kernel: stream_leaves_kernel (SHA-256 of every 2048-byte leaf of both fragments), ALU-bound like the DCT path
