@@ -389,3 +389,58 @@ def defragment_dct_packed(priv, pub, w, h, c, k, ac_bits, key, nonce, expected=N
                                          out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(fl))
     assert rc == 0, rc
     return out, int(fl.value)
+
+
+# ------------------------------------------------------------------------------------------ tiled DWT design (feds_oracle_tiled.c)
+def tiled_forward(tile) -> np.ndarray:
+    """8x8 uint8 tile -> its 64 coefficients in level order (DESIGN.md 2.5 T2)"""
+    t, p = _u8(np.ascontiguousarray(tile, dtype=np.uint8).reshape(64))
+    out = np.zeros(64, dtype=np.int32)
+    lib().orc_tiled_forward(p, out.ctypes.data_as(C.POINTER(C.c_int32)))
+    return out
+
+
+def tiled_inverse(coef) -> np.ndarray:
+    cf = np.ascontiguousarray(coef, dtype=np.int32).reshape(64)
+    out = np.zeros(64, dtype=np.uint8)
+    lib().orc_tiled_inverse(cf.ctypes.data_as(C.POINTER(C.c_int32)), out.ctypes.data_as(C.POINTER(C.c_uint8)))
+    return out.reshape(8, 8)
+
+
+def tiled_pack(coef):
+    """-> (level-1 bytes[5], level-2 bytes[16], level-3 bytes[60]) or None when a value does not fit its field"""
+    cf = np.ascontiguousarray(coef, dtype=np.int32).reshape(64)
+    l1, l2, l3 = (C.c_uint8 * 5)(), (C.c_uint8 * 16)(), (C.c_uint8 * 60)()
+    rc = lib().orc_tiled_pack(cf.ctypes.data_as(C.POINTER(C.c_int32)), l1, l2, l3)
+    return None if rc else (bytes(l1), bytes(l2), bytes(l3))
+
+
+def tiled_private_bytes(w, h, c):
+    return (w // 8) * (h // 8) * c * 21
+
+
+def tiled_public_bytes(w, h, c):
+    return (w // 8) * (h // 8) * c * 60
+
+
+def fragment_tiled(image, key, nonce, leaf_bytes=LEAF_BYTES, fanout=FANOUT):
+    img, h, w, c = _img(image)
+    priv = np.zeros(tiled_private_bytes(w, h, c), dtype=np.uint8)
+    pub = np.zeros(tiled_public_bytes(w, h, c), dtype=np.uint8)
+    dg = (C.c_uint8 * 64)()
+    rc = lib().orc_fragment_tiled(img.ctypes.data_as(C.POINTER(C.c_uint8)), w, h, c, _key(key), _key(nonce), C.c_uint64(leaf_bytes), fanout,
+                                  priv.ctypes.data_as(C.POINTER(C.c_uint8)), pub.ctypes.data_as(C.POINTER(C.c_uint8)), dg)
+    assert rc == 0, rc
+    return priv, pub, bytes(dg)
+
+
+def defragment_tiled(priv, pub, w, h, c, key, nonce, expected=None, leaf_bytes=LEAF_BYTES, fanout=FANOUT):
+    pa, pp = _u8(priv)
+    qa, qp = _u8(pub)
+    out = np.zeros((h, w, c), dtype=np.uint8)
+    fl = C.c_uint32(0)
+    exp = (C.c_uint8 * 64).from_buffer_copy(bytes(expected)) if expected is not None else None
+    rc = lib().orc_defragment_tiled(pp, qp, w, h, c, _key(key), _key(nonce), C.c_uint64(leaf_bytes), fanout, exp,
+                                    out.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(fl))
+    assert rc == 0, rc
+    return out, int(fl.value)

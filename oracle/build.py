@@ -1,4 +1,4 @@
-"""Build the CPU oracle (oracle/feds_oracle.c, feds_oracle_strong.c, feds_oracle_packed.c) into oracle/libfeds_oracle.so with gcc.
+"""Build the CPU oracle (oracle/feds_oracle.c, feds_oracle_strong.c, feds_oracle_packed.c, feds_oracle_tiled.c) into oracle/libfeds_oracle.so with gcc.
 
 TEST INFRASTRUCTURE. `python -m oracle.build` or `oracle.build.build()`; called by tests/conftest.py,
 `__graft_entry__.build()` and bench.py's cpu_baseline leg. Plain `gcc -O2`, no SIMD flags, libm only.
@@ -7,7 +7,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRCS = [os.path.join(HERE, "feds_oracle.c"), os.path.join(HERE, "feds_oracle_strong.c"), os.path.join(HERE, "feds_oracle_packed.c")]
+SRCS = [os.path.join(HERE, "feds_oracle.c"), os.path.join(HERE, "feds_oracle_strong.c"), os.path.join(HERE, "feds_oracle_packed.c"), os.path.join(HERE, "feds_oracle_tiled.c")]
 LIB = os.path.join(HERE, "libfeds_oracle.so")
 
 
