@@ -263,6 +263,37 @@ feds_status feds_defragment_dct_host(const uint8_t *h_private, const uint8_t *h_
                                      size_t scratch_bytes, feds_stream_t *streams, int n_streams, unsigned flags);
 
 /*
+ * The report's own DWT design (PAPER.md 6.9.3-6.9.4, Figure 18; byte format: DESIGN.md 2.5): every 8x8 tile of every
+ * channel plane gets two levels of the integer Le Gall 5/3 transform. "Level 1" (the four LL2 coefficients, 40 bits) is protected by
+ * AES-128-CTR; "level 2" (HL2, LH2, HH2: 124 bits) is XORed with SHA-256(level 1 || key || nonce); "level 3" (HL1, LH1, HH1: 480 bits)
+ * with SHA-512(level 2 || key || nonce); fields of 10 bits, 11 for HH2.
+ *   d_private: feds_dwt_tiles_private_bytes() = 21 bytes per tile: [16 bytes of protected level 2 per tile] then [5 bytes of level 1
+ *              per tile, all tiles as one AES-128-CTR message]
+ *   d_public : feds_dwt_tiles_public_bytes() = 60 bytes per tile (protected level 3); tiles in the order channel, tile row, tile column
+ *   d_digests: 64 bytes, stream Merkle roots of the two fragments as stored (2048-byte leaves, as the DWT path)
+ *   workspace: feds_dwt_tiles_workspace_bytes() per image. w, h multiples of 8. The inverse is exact.
+ */
+size_t feds_dwt_tiles_private_bytes(int w, int h, int c);
+size_t feds_dwt_tiles_public_bytes(int w, int h, int c);
+size_t feds_dwt_tiles_workspace_bytes(int w, int h, int c);
+feds_status feds_fragment_dwt_tiles(const uint8_t *d_image, int w, int h, int c, const uint8_t key[16], const uint8_t nonce[16],
+                                    uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests, void *d_workspace,
+                                    size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_defragment_dwt_tiles(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c,
+                                      const uint8_t key[16], const uint8_t nonce[16], const uint8_t *d_expected_digests,
+                                      uint8_t *d_image_out, uint32_t *d_verify_flags, void *d_workspace,
+                                      size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_fragment_dwt_tiles_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c,
+                                          const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private,
+                                          size_t private_stride, uint8_t *d_public, size_t public_stride, uint8_t *d_digests,
+                                          void *d_workspace, size_t workspace_bytes, feds_stream_t stream);
+feds_status feds_defragment_dwt_tiles_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public,
+                                            size_t public_stride, int n_images, int w, int h, int c, const uint8_t key[16],
+                                            const uint8_t *d_nonces, const uint8_t *d_expected_digests, uint8_t *d_images_out,
+                                            size_t image_stride, uint32_t *d_verify_flags, void *d_workspace,
+                                            size_t workspace_bytes, feds_stream_t stream);
+
+/*
  * Stream primitives: the two cryptographic steps of the path on a plain byte stream in device memory.
  *
  * feds_aes128_ctr — step 4 alone: d_out[i] = d_in[i] XOR keystream[i] over n_bytes bytes, counter block of the j-th

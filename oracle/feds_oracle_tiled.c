@@ -17,7 +17,7 @@
  *       stream (fields LSB first) padded with zero bits to whole bytes: 5, 16 (124 bits) and 60 bytes.
  *   T4  K2 = SHA-256(level-1 bytes || key || IV), K3 = SHA-512(level-2 bytes || key || IV), plaintext bytes as packed (pad bits zero),
  *       IV = the image's 16-byte nonce; stored level 2 = its 16 bytes XOR K2[0..15], stored level 3 = its 60 bytes XOR K3[0..59].
- *   T5  private fragment = [level-1 bytes of all tiles, 5 per tile, as ONE AES-128-CTR message] || [stored level-2 bytes, 16 per tile];
+ *   T5  private fragment = [stored level-2 bytes, 16 per tile] || [level-1 bytes of all tiles, 5 per tile, as ONE AES-128-CTR message];
  *       public fragment = stored level-3 bytes, 60 per tile. Tile order: channel, tile row, tile column. 21 private bytes per 64
  *       pixels = 32.8 % ("at most 32%"), 81 bytes in all = 126.6 % ("about 26% more"; 4 pad bits per tile more than 644 bits).
  *   T6  digests: the stream Merkle layout of DESIGN.md 2.2 (2048-byte leaves, fan-out 16) over each fragment as stored.
@@ -149,7 +149,7 @@ int orc_fragment_tiled(const uint8_t *image, int w, int h, int c, const uint8_t 
     if (check_dims(w, h, c)) return -1;
     int ntr = h / 8, ntc = w / 8;
     uint64_t T = (uint64_t)c * ntr * ntc;
-    uint8_t *secA = priv, *secB = priv + 5 * T;
+    uint8_t *secB = priv, *secA = priv + 16 * T;   /* T5 */
     for (int ch = 0; ch < c; ch++)
         for (int tr = 0; tr < ntr; tr++)
             for (int tc = 0; tc < ntc; tc++) {
@@ -188,9 +188,9 @@ int orc_defragment_tiled(const uint8_t *priv, const uint8_t *pub, int w, int h, 
     }
     uint8_t *secA = (uint8_t *)malloc(5 * T ? 5 * T : 1);
     if (!secA) return -3;
-    memcpy(secA, priv, 5 * T);
+    memcpy(secA, priv + 16 * T, 5 * T);
     orc_aes128_ctr_xor(key, nonce, 0, secA, 5 * T);
-    const uint8_t *secB = priv + 5 * T;
+    const uint8_t *secB = priv;
     for (int ch = 0; ch < c; ch++)
         for (int tr = 0; tr < ntr; tr++)
             for (int tc = 0; tc < ntc; tc++) {

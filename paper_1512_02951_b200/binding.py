@@ -35,6 +35,8 @@ SYMBOLS = [
     "feds_defragment_dct_strong_batch", "feds_debug_strong_basis_host",
     "feds_dct_packed_private_bytes", "feds_dct_packed_workspace_bytes", "feds_fragment_dct_packed", "feds_defragment_dct_packed",
     "feds_fragment_dct_packed_batch", "feds_defragment_dct_packed_batch",
+    "feds_dwt_tiles_private_bytes", "feds_dwt_tiles_public_bytes", "feds_dwt_tiles_workspace_bytes", "feds_fragment_dwt_tiles",
+    "feds_defragment_dwt_tiles", "feds_fragment_dwt_tiles_batch", "feds_defragment_dwt_tiles_batch",
     "feds_debug_sha256_host", "feds_debug_aes128_host", "feds_debug_dct8x8_host", "feds_debug_zigzag_host", "feds_debug_launch_count",
 ]
 
@@ -76,6 +78,13 @@ def _load():
     for name in ["feds_dct_packed_private_bytes", "feds_dct_packed_workspace_bytes"]:
         getattr(lib, name).restype = sz
         getattr(lib, name).argtypes = [i, i, i, i, i]
+    for name in ["feds_dwt_tiles_private_bytes", "feds_dwt_tiles_public_bytes", "feds_dwt_tiles_workspace_bytes"]:
+        getattr(lib, name).restype = sz
+        getattr(lib, name).argtypes = [i, i, i]
+    lib.feds_fragment_dwt_tiles.argtypes = [vp, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
+    lib.feds_defragment_dwt_tiles.argtypes = [vp, vp, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
+    lib.feds_fragment_dwt_tiles_batch.argtypes = [vp, i, sz, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, vp]
+    lib.feds_defragment_dwt_tiles_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, u8p, vp, vp, vp, sz, vp, vp, sz, vp]
     lib.feds_fragment_dct_packed.argtypes = [vp, i, i, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
     lib.feds_defragment_dct_packed.argtypes = [vp, vp, i, i, i, i, i, u8p, u8p, vp, vp, vp, vp, sz, vp]
     lib.feds_fragment_dct_packed_batch.argtypes = [vp, i, sz, i, i, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, vp]
@@ -106,7 +115,8 @@ def _load():
                  "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
                  "feds_fragment_dct_host", "feds_defragment_dct_host", "feds_fragment_dct_strong", "feds_defragment_dct_strong",
                  "feds_fragment_dct_strong_batch", "feds_defragment_dct_strong_batch", "feds_fragment_dct_packed", "feds_defragment_dct_packed",
-                 "feds_fragment_dct_packed_batch", "feds_defragment_dct_packed_batch",
+                 "feds_fragment_dct_packed_batch", "feds_defragment_dct_packed_batch", "feds_fragment_dwt_tiles", "feds_defragment_dwt_tiles",
+                 "feds_fragment_dwt_tiles_batch", "feds_defragment_dwt_tiles_batch",
                  "feds_aes128_ctr", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt"]:
         getattr(lib, name).restype = i
     return lib
@@ -295,6 +305,58 @@ class PackedBatch:
                                                     self.h, self.c, self.k, self.ac_bits, _k16(key), _ptr(d_nonces), _ptr(expected),
                                                     _ptr(images_out), self.image_bytes, _ptr(self.flags_out), _ptr(self.ws),
                                                     self.ws.numel(), _stream(stream)), "feds_defragment_dct_packed_batch")
+
+
+def fragment_dwt_tiles(image, key, nonce, stream=None):
+    """feds_fragment_dwt_tiles: the report's tiled DWT design -> (private 21 B/tile, public 60 B/tile, digests[64])"""
+    image, w, h, c = _hwc(image)
+    dev = image.device
+    pvb, pbb = lib.feds_dwt_tiles_private_bytes(w, h, c), lib.feds_dwt_tiles_public_bytes(w, h, c)
+    priv, pub, dg = _u8(pvb, dev), _u8(pbb, dev), _u8(64, dev)
+    ws = _u8(lib.feds_dwt_tiles_workspace_bytes(w, h, c), dev)
+    _on_stream(stream, priv, pub, dg, ws)
+    _check(lib.feds_fragment_dwt_tiles(_ptr(image), w, h, c, _k16(key), _k16(nonce), _ptr(priv), _ptr(pub), _ptr(dg), _ptr(ws), ws.numel(),
+                                       _stream(stream)), "feds_fragment_dwt_tiles")
+    return priv[:pvb], pub[:pbb], dg
+
+
+def defragment_dwt_tiles(priv, pub, w, h, c, key, nonce, expected=None, stream=None):
+    dev = priv.device
+    out = torch.empty((h, w, c), dtype=torch.uint8, device=dev)
+    flags = torch.zeros(1, dtype=torch.int32, device=dev) if expected is not None else None
+    ws = _u8(lib.feds_dwt_tiles_workspace_bytes(w, h, c), dev)
+    _on_stream(stream, out, flags, ws)
+    _check(lib.feds_defragment_dwt_tiles(_ptr(priv), _ptr(pub), w, h, c, _k16(key), _k16(nonce), _ptr(expected), _ptr(out), _ptr(flags),
+                                         _ptr(ws), ws.numel(), _stream(stream)), "feds_defragment_dwt_tiles")
+    return out, flags
+
+
+class TilesBatch:
+    """Pre-allocated buffers for feds_fragment_dwt_tiles_batch / feds_defragment_dwt_tiles_batch on n images of one shape."""
+
+    def __init__(self, n, w, h, c, device="cuda"):
+        self.n, self.w, self.h, self.c = n, w, h, c
+        self.image_bytes = w * h * c
+        self.priv_bytes = lib.feds_dwt_tiles_private_bytes(w, h, c)
+        self.pub_bytes = lib.feds_dwt_tiles_public_bytes(w, h, c)
+        self.priv_stride = (self.priv_bytes + 15) // 16 * 16
+        self.pub_stride = (self.pub_bytes + 15) // 16 * 16
+        self.priv = _u8(n * self.priv_stride, device)
+        self.pub = _u8(n * self.pub_stride, device)
+        self.digests = _u8(n * 64, device)
+        self.ws = _u8(n * lib.feds_dwt_tiles_workspace_bytes(w, h, c), device)
+        self.flags_out = torch.zeros(n, dtype=torch.int32, device=device)
+
+    def fragment(self, images, key, d_nonces, stream=None):
+        _check(lib.feds_fragment_dwt_tiles_batch(_ptr(images), self.n, self.image_bytes, self.w, self.h, self.c, _k16(key), _ptr(d_nonces),
+                                                 _ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, _ptr(self.digests),
+                                                 _ptr(self.ws), self.ws.numel(), _stream(stream)), "feds_fragment_dwt_tiles_batch")
+
+    def defragment(self, images_out, key, d_nonces, expected=None, stream=None):
+        _check(lib.feds_defragment_dwt_tiles_batch(_ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, self.n, self.w, self.h,
+                                                   self.c, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out), self.image_bytes,
+                                                   _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), _stream(stream)),
+               "feds_defragment_dwt_tiles_batch")
 
 
 def verify_dct(priv, pub, w, h, c, k, expected, stream=None, workspace=None):

@@ -536,6 +536,88 @@ feds_status defragment_packed_impl(const uint8_t *d_private, size_t private_stri
     return launch_defragment_packed(p, c, plain, plain_stride, stream, d_expected == nullptr);
 }
 
+// ---------------------------------------------------------------------------------------------- tiled DWT design
+DwtPlan tiles_plan(int w, int h, int c) {
+    DwtPlan pl{};
+    const size_t T = (size_t)(w / 8) * (h / 8) * c;
+    pl.priv_b = 21 * T;
+    pl.pub_b = 60 * T;
+    pl.priv_nl = (unsigned)((pl.priv_b + DWT_LEAF_BYTES - 1) / DWT_LEAF_BYTES);
+    pl.pub_nl = (unsigned)((pl.pub_b + DWT_LEAF_BYTES - 1) / DWT_LEAF_BYTES);
+    pl.planes_bytes = 0;
+    pl.priv_tree = std::max<size_t>(tree_bytes(pl.priv_nl), 32);
+    pl.pub_tree = std::max<size_t>(tree_bytes(pl.pub_nl), 32);
+    pl.per_image = round_up(round_up(pl.priv_tree, 256) + round_up(pl.pub_tree, 256) + 64, 256);
+    return pl;
+}
+feds_status check_tiles_args(int n_images, int w, int h, int c) {
+    if (!dct_dims_ok(w, h)) return FEDS_ERR_BAD_DIMS;
+    if (!chan_ok(c) || n_images < 1) return FEDS_ERR_BAD_PARAM;
+    return FEDS_OK;
+}
+void fill_tiles_params(DctParams &p, int n_images, int w, int h, const uint8_t key[16], const uint8_t *d_nonces, const uint8_t *nonce_host) {
+    memset(&p, 0, sizeof p);
+    p.n_images = n_images; p.w = w; p.h = h;
+    p.nbr = h / 8; p.nbc = w / 8;
+    p.one = 1u;
+    p.d_nonces = d_nonces;
+    if (nonce_host) nonce_to_be(nonce_host, p.nonce_be);
+    aes128_expand_key_host(key, p.rk, h_aes);
+}
+
+feds_status fragment_tiles_impl(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c, const uint8_t key[16],
+                                const uint8_t *nonce_host, const uint8_t *d_nonces, uint8_t *d_private, size_t private_stride,
+                                uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
+                                cudaStream_t stream) {
+    feds_status st = check_tiles_args(n_images, w, h, c);
+    if (st != FEDS_OK) return st;
+    if (!d_images || !key || (!nonce_host && !d_nonces) || !d_private || !d_public || !d_digests || !d_workspace) return FEDS_ERR_NULL_POINTER;
+    const DwtPlan pl = tiles_plan(w, h, c);
+    if (image_stride < (size_t)w * h * c || private_stride < pl.priv_b || public_stride < pl.pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images) || misaligned(d_private) || misaligned(d_public) || misaligned(d_digests) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    if (workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+    DctParams p;
+    fill_tiles_params(p, n_images, w, h, key, d_nonces, nonce_host);
+    p.images = d_images; p.image_stride = image_stride;
+    p.priv = d_private; p.priv_stride = private_stride;
+    p.pub = d_public; p.pub_stride = public_stride;
+    st = launch_fragment_dwt_tiles(p, c, stream);
+    if (st != FEDS_OK) return st;
+    return dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, static_cast<uint8_t *>(d_workspace), d_digests, stream);
+}
+
+feds_status defragment_tiles_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride, int n_images,
+                                  int w, int h, int c, const uint8_t key[16], const uint8_t *nonce_host, const uint8_t *d_nonces,
+                                  const uint8_t *d_expected, uint8_t *d_images_out, size_t image_stride, uint32_t *d_flags, void *d_workspace,
+                                  size_t workspace_bytes, cudaStream_t stream) {
+    feds_status st = check_tiles_args(n_images, w, h, c);
+    if (st != FEDS_OK) return st;
+    if (!d_private || !d_public || !key || (!nonce_host && !d_nonces) || !d_images_out || (d_expected && (!d_flags || !d_workspace)))
+        return FEDS_ERR_NULL_POINTER;
+    const DwtPlan pl = tiles_plan(w, h, c);
+    if (image_stride < (size_t)w * h * c || private_stride < pl.priv_b || public_stride < pl.pub_b) return FEDS_ERR_BAD_PARAM;
+    if (misaligned(d_images_out) || misaligned(d_private) || misaligned(d_public) || misaligned(d_expected) || misaligned(d_workspace) ||
+        misaligned(d_nonces) || (n_images > 1 && ((image_stride | private_stride | public_stride) & 15u)))
+        return FEDS_ERR_MISALIGNED;
+    if (d_expected) {
+        if (workspace_bytes < pl.per_image * (size_t)n_images) return FEDS_ERR_WORKSPACE_TOO_SMALL;
+        uint8_t *ws = static_cast<uint8_t *>(d_workspace);
+        uint8_t *roots = ws + pl.per_image * (size_t)n_images - 64 * (size_t)n_images;
+        st = dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, ws, roots, stream);
+        if (st != FEDS_OK) return st;
+        st = launch_compare_digests(roots, d_expected, d_flags, n_images, stream);
+        if (st != FEDS_OK) return st;
+    }
+    DctParams p;
+    fill_tiles_params(p, n_images, w, h, key, d_nonces, nonce_host);
+    p.images_out = d_images_out; p.image_stride = image_stride;
+    p.priv = const_cast<uint8_t *>(d_private); p.priv_stride = private_stride;
+    p.pub = const_cast<uint8_t *>(d_public); p.pub_stride = public_stride;
+    return launch_defragment_dwt_tiles(p, c, stream);
+}
+
 }  // namespace
 
 // =================================================================================================== C ABI
@@ -783,6 +865,44 @@ feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, i
     const feds_status st = dwt_digests(d_private, pl.priv_b, d_public, pl.pub_b, 1, pl, ws + pl.planes_bytes, roots, stream);
     if (st != FEDS_OK) return st;
     return launch_compare_digests(roots, d_expected_digests, d_verify_flags, 1, stream);
+}
+
+// ------------------------------------------------------------------------------------------------ tiled DWT design
+size_t feds_dwt_tiles_private_bytes(int w, int h, int c) { return (dct_dims_ok(w, h) && chan_ok(c)) ? tiles_plan(w, h, c).priv_b : 0; }
+size_t feds_dwt_tiles_public_bytes(int w, int h, int c) { return (dct_dims_ok(w, h) && chan_ok(c)) ? tiles_plan(w, h, c).pub_b : 0; }
+size_t feds_dwt_tiles_workspace_bytes(int w, int h, int c) { return (dct_dims_ok(w, h) && chan_ok(c)) ? tiles_plan(w, h, c).per_image : 0; }
+
+feds_status feds_fragment_dwt_tiles(const uint8_t *d_image, int w, int h, int c, const uint8_t key[16], const uint8_t nonce[16],
+                                    uint8_t *d_private, uint8_t *d_public, uint8_t *d_digests, void *d_workspace, size_t workspace_bytes,
+                                    feds_stream_t stream) {
+    if (!nonce) return check_tiles_args(1, w, h, c) != FEDS_OK ? check_tiles_args(1, w, h, c) : FEDS_ERR_NULL_POINTER;
+    return fragment_tiles_impl(d_image, 1, (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0), w, h, c, key, nonce, nullptr, d_private,
+                               feds_dwt_tiles_private_bytes(w, h, c), d_public, feds_dwt_tiles_public_bytes(w, h, c), d_digests, d_workspace,
+                               workspace_bytes, stream);
+}
+feds_status feds_fragment_dwt_tiles_batch(const uint8_t *d_images, int n_images, size_t image_stride, int w, int h, int c,
+                                          const uint8_t key[16], const uint8_t *d_nonces, uint8_t *d_private, size_t private_stride,
+                                          uint8_t *d_public, size_t public_stride, uint8_t *d_digests, void *d_workspace,
+                                          size_t workspace_bytes, feds_stream_t stream) {
+    if (!d_nonces) return check_tiles_args(n_images, w, h, c) != FEDS_OK ? check_tiles_args(n_images, w, h, c) : FEDS_ERR_NULL_POINTER;
+    return fragment_tiles_impl(d_images, n_images, image_stride, w, h, c, key, nullptr, d_nonces, d_private, private_stride, d_public,
+                               public_stride, d_digests, d_workspace, workspace_bytes, stream);
+}
+feds_status feds_defragment_dwt_tiles(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, const uint8_t key[16],
+                                      const uint8_t nonce[16], const uint8_t *d_expected_digests, uint8_t *d_image_out,
+                                      uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, feds_stream_t stream) {
+    if (!nonce) return check_tiles_args(1, w, h, c) != FEDS_OK ? check_tiles_args(1, w, h, c) : FEDS_ERR_NULL_POINTER;
+    return defragment_tiles_impl(d_private, feds_dwt_tiles_private_bytes(w, h, c), d_public, feds_dwt_tiles_public_bytes(w, h, c), 1, w, h, c, key,
+                                 nonce, nullptr, d_expected_digests, d_image_out, (size_t)(w > 0 ? w : 0) * (h > 0 ? h : 0) * (c > 0 ? c : 0),
+                                 d_verify_flags, d_workspace, workspace_bytes, stream);
+}
+feds_status feds_defragment_dwt_tiles_batch(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                            int n_images, int w, int h, int c, const uint8_t key[16], const uint8_t *d_nonces,
+                                            const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                            uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, feds_stream_t stream) {
+    if (!d_nonces) return check_tiles_args(n_images, w, h, c) != FEDS_OK ? check_tiles_args(n_images, w, h, c) : FEDS_ERR_NULL_POINTER;
+    return defragment_tiles_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, key, nullptr, d_nonces,
+                                 d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, stream);
 }
 
 // ------------------------------------------------------------------------------------------------ stream primitives

@@ -64,6 +64,9 @@ void strong_basis_host(int32_t out[64 * 64]);
 feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t stream, bool profile);
 feds_status launch_defragment_packed(const DctParams &p, int c, const uint8_t *plain, size_t plain_stride, cudaStream_t stream, bool profile);
 feds_status launch_packed_private_leaves(const DctParams &p, int c, cudaStream_t stream);
+// ---- feds_k_dwt_tiles.cu: the report's tiled DWT design (one thread per 8x8 tile; the profiling events bracket the kernel)
+feds_status launch_fragment_dwt_tiles(const DctParams &p, int c, cudaStream_t stream);
+feds_status launch_defragment_dwt_tiles(const DctParams &p, int c, cudaStream_t stream);
 // ---- feds_k_hash.cu: Merkle upper levels, stream leaves, AES-CTR stream, digest compare
 feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
                      int skip_odd, cudaStream_t stream);

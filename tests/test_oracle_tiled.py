@@ -80,7 +80,7 @@ def test_fragment_layout_keystreams_and_round_trip(w, h, c):
         priv, pub, dg = oracle.fragment_tiled(img, key, nonce)
         T = (w // 8) * (h // 8) * c
         assert priv.size == 21 * T and pub.size == 60 * T
-        sec_a = oracle.aes128_ctr_xor(key, nonce, priv[:5 * T].tobytes())      # T5: level 1 of all tiles is one CTR message
+        sec_a = oracle.aes128_ctr_xor(key, nonce, priv[16 * T:].tobytes())     # T5: level 1 of all tiles is one CTR message, behind level 2
         ntr, ntc = h // 8, w // 8
         for t in sorted({0, T // 2, T - 1}):
             ch, rem = divmod(t, ntr * ntc)
@@ -89,7 +89,7 @@ def test_fragment_layout_keystreams_and_round_trip(w, h, c):
             l1 = sec_a[5 * t:5 * t + 5]
             assert py_fields(l1, 0, 4) == list(coef[0:4])
             k2 = hashlib.sha256(l1 + key + nonce).digest()                       # T4
-            l2 = bytes(a ^ b_ for a, b_ in zip(priv[5 * T + 16 * t:5 * T + 16 * t + 16].tobytes(), k2[:16]))
+            l2 = bytes(a ^ b_ for a, b_ in zip(priv[16 * t:16 * t + 16].tobytes(), k2[:16]))
             assert py_fields(l2, 4, 16) == list(coef[4:16]) and l2[15] >> 4 == 0
             k3 = hashlib.sha512(l2 + key + nonce).digest()
             l3 = bytes(a ^ b_ for a, b_ in zip(pub[60 * t:60 * t + 60].tobytes(), k3[:60]))
@@ -97,7 +97,7 @@ def test_fragment_layout_keystreams_and_round_trip(w, h, c):
         assert dg[:32] == oracle.merkle_stream(priv) and dg[32:] == oracle.merkle_stream(pub)   # T6 (merkle_stream is pinned by hashlib)
         rec, fl = oracle.defragment_tiled(priv, pub, w, h, c, key, nonce, expected=dg)
         assert fl == 0 and (rec == img).all()                                                   # no error at all
-        p2 = priv.copy(); p2[3] ^= 1
+        p2 = priv.copy(); p2[16 * T + 3] ^= 1
         q2 = pub.copy(); q2[-1] ^= 1
         assert oracle.defragment_tiled(p2, pub, w, h, c, key, nonce, expected=dg)[1] == 1
         assert oracle.defragment_tiled(priv, q2, w, h, c, key, nonce, expected=dg)[1] == 2
