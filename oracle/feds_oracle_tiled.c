@@ -186,7 +186,7 @@ int orc_defragment_tiled(const uint8_t *priv, const uint8_t *pub, int w, int h, 
         if (memcmp(dg + 32, expected + 32, 32)) fl |= 2u;
         if (flags) *flags = fl;
     }
-    uint8_t *secA = (uint8_t *)malloc(5 * T ? 5 * T : 1);
+    uint8_t *secA = (uint8_t *)malloc(T ? 5 * T : 1);
     if (!secA) return -3;
     memcpy(secA, priv + 16 * T, 5 * T);
     orc_aes128_ctr_xor(key, nonce, 0, secA, 5 * T);

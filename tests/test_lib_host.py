@@ -150,3 +150,38 @@ def test_strong_level_basis_table_equals_the_oracles():
     out = np.zeros(4096, dtype=np.int32)
     binding.lib.feds_debug_strong_basis_host(out.ctypes.data)
     assert (out.reshape(64, 64) == oracle.strong_basis()).all()
+
+
+def test_sizes_and_argument_errors_of_the_widened_entry_points(b):
+    """strong level, packed storage, tiled DWT design: sizes as the formats of DESIGN.md 2.3-2.5 define them, and
+    argument errors reported before anything is enqueued (no GPU needed: every call below must fail in validation)."""
+    L = b.lib
+    key = bytes(16)
+    ok = C.c_void_p(0x1000)
+    assert L.feds_dct_strong_public_bytes(1920, 1080, 3) == 1920 * 1080 * 3 and L.feds_dct_strong_public_bytes(12, 16, 1) == 0
+    # P:599: 66 bytes per 8 blocks (11-bit), 51 (8-bit) at k = 5; a ragged group rounds up to whole bytes
+    assert L.feds_dct_packed_private_bytes(512, 512, 1, 5, 11) == 512 * 512 * 66 // 512
+    assert L.feds_dct_packed_private_bytes(512, 512, 1, 5, 8) == 512 * 512 * 51 // 512
+    assert L.feds_dct_packed_private_bytes(72, 8, 1, 5, 11) == 66 + 9 and L.feds_dct_packed_private_bytes(64, 8, 1, 5, 9) == 0
+    assert L.feds_dct_packed_workspace_bytes(64, 8, 1, 5, 11) >= L.feds_workspace_bytes(64, 8, 1, 5, 0) + 66
+    assert L.feds_dwt_tiles_private_bytes(512, 512, 1) == 4096 * 21 and L.feds_dwt_tiles_public_bytes(512, 512, 1) == 4096 * 60   # P:820
+    assert L.feds_dwt_tiles_private_bytes(12, 8, 1) == 0 and L.feds_dwt_tiles_workspace_bytes(512, 512, 1) % 256 == 0
+    f = L.feds_fragment_dct_strong
+    assert f(None, 16, 16, 1, 3, key, key, ok, ok, ok, ok, 1 << 20, None) == 1
+    assert f(ok, 12, 16, 1, 3, key, key, ok, ok, ok, ok, 1 << 20, None) == 2
+    assert f(ok, 16, 16, 1, 64, key, key, ok, ok, ok, ok, 1 << 20, None) == 3
+    assert f(ok, 64, 64, 1, 3, key, key, ok, ok, ok, ok, 8, None) == 4
+    assert f(ok, 16, 16, 1, 3, key, key, C.c_void_p(0x1004), ok, ok, ok, 1 << 20, None) == 6
+    g = L.feds_fragment_dct_packed
+    assert g(ok, 16, 16, 1, 3, 11, key, key, None, ok, ok, ok, 1 << 20, None) == 1
+    assert g(ok, 16, 20, 1, 3, 11, key, key, ok, ok, ok, ok, 1 << 20, None) == 2
+    assert g(ok, 16, 16, 1, 3, 10, key, key, ok, ok, ok, ok, 1 << 20, None) == 3            # ac_bits must be 11 or 8
+    assert g(ok, 64, 64, 1, 3, 8, key, key, ok, ok, ok, ok, 8, None) == 4
+    h = L.feds_defragment_dct_packed
+    assert h(ok, ok, 16, 16, 1, 3, 11, key, key, ok, ok, None, ok, 1 << 20, None) == 1      # expected digests without a flag word
+    t = L.feds_fragment_dwt_tiles
+    assert t(ok, 16, 12, 1, key, key, ok, ok, ok, ok, 1 << 20, None) == 2
+    assert t(ok, 16, 16, 2, key, key, ok, ok, ok, ok, 1 << 20, None) == 3
+    assert t(ok, 16, 16, 1, key, None, ok, ok, ok, ok, 1 << 20, None) == 1
+    assert t(ok, 64, 64, 1, key, key, ok, ok, ok, ok, 8, None) == 4
+    assert t(ok, 16, 16, 1, key, key, ok, C.c_void_p(0x1008), ok, ok, 1 << 20, None) == 6
