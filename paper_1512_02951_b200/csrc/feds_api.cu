@@ -102,6 +102,7 @@ void fill_dct_params(DctParams &p, int n_images, int w, int h, int c, int k, con
     p.leaves_per_image = (unsigned)c * p.nbr * p.nlr;
     p.total_leaves = (unsigned long long)p.leaves_per_image * n_images;
     p.one = 1u;
+    p.c128 = 128u;
     p.pub_words = strong ? 16 : 63 - k;
     p.priv_words = k + 1;
     (void)digest;

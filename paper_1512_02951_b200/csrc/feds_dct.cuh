@@ -28,6 +28,7 @@ struct DctParams {
     unsigned leaves_per_image;  // C * nbr * nlr
     unsigned long long total_leaves;
     uint32_t one;     // = 1, opaque to the compiler (see sha256_compress_rolled_fma)
+    uint32_t c128;    // = 128, opaque to the compiler (rep_lookup, feds_aes_rep.cuh)
     int pub_words;      // 32-bit words per block in the public fragment: 63 - k (first level) or 16 (strong level: 64 pixel bytes)
     int priv_words;     // 32-bit words per block in the private fragment for the leaf-hash kernels: k + 1, or 0 = skip (packed storage)
     // packed integer storage (feds_dct_packed.cuh)

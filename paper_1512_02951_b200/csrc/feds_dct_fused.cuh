@@ -29,6 +29,9 @@ constexpr int FU_UNIT_BLOCKS = 32 * G_BLOCKS;   // 32 leaves of 8 blocks: one ha
 constexpr int FU_TILE_WARPS = 8;                // two warpgroups (setmaxnreg acts on aligned groups of 4 warps)
 constexpr int FU_HASH_REGS = 72;
 constexpr int FU_CTL_OFFSET = 128;              // progress words sit behind the groups' mbarriers inside TMA_BAR_BYTES
+// AES tables of the tile role: the four-table layout (feds_aes_rep.cuh), 128 KB: one ALU-pipe instruction per lookup instead of
+// three -- in this kernel the ALU pipe is the contended resource, and the tile role's AES was 40 % of its ALU-pipe work
+constexpr size_t FU_TABLE_BYTES = (size_t)REP4_TABLE_WORDS * 4;
 
 template <int C, int HW> struct FuShape {
     static constexpr int THREADS = (HW + FU_TILE_WARPS) * 32;
@@ -37,7 +40,7 @@ template <int C, int HW> struct FuShape {
     // registers: HW * 72 + 8 * TILE_REGS <= (HW + 8) * (registers per thread at launch)
     static constexpr int TILE_REGS = (HW >= 16) ? 96 : 128;
 };
-template <int C> __host__ __device__ inline size_t fu_smem_bytes(int k, int np) { return tma_smem_bytes<C>(k, np); }
+template <int C> __host__ __device__ inline size_t fu_smem_bytes(int k, int np) { return tma_smem_bytes<C>(k, np, FU_TABLE_BYTES); }
 template <int C> __host__ __device__ inline bool fu_shape_ok(int w) { return tma_shape_ok<C>(w) && ((w / 8) % G_BLOCKS) == 0; }
 
 __device__ __forceinline__ int fu_ld_volatile(const int *p) {
@@ -148,7 +151,7 @@ __device__ __forceinline__ void fu_hash_role(const DctParams &p, const FuWork &W
 
 // ------------------------------------------------------------------------------------------------------------ TILE roles
 template <int C, int V, int NP, int TPU>
-__device__ __forceinline__ void fu_fragment_tiles(const DctParams &p, const FuWork &W, const T0Lane &sT, const TmaGroup<C> &G, int *progress) {
+__device__ __forceinline__ void fu_fragment_tiles(const DctParams &p, const FuWork &W, const RepAes &sT, const TmaGroup<C> &G, int *progress) {
     using S = TmaShape<C>;
     const unsigned s_end = TPU * W.n_units;
     const int gid = G.gid, tid = G.tid;
@@ -182,7 +185,7 @@ __device__ __forceinline__ void fu_fragment_tiles(const DctParams &p, const FuWo
     }
 }
 template <int C, int V, int NP, int TPU>
-__device__ __forceinline__ void fu_defragment_tiles(const DctParams &p, const FuWork &W, const T0Lane &sT, const TmaGroup<C> &G) {
+__device__ __forceinline__ void fu_defragment_tiles(const DctParams &p, const FuWork &W, const RepAes &sT, const TmaGroup<C> &G) {
     const unsigned s_end = TPU * W.n_units;
     const int gid = G.gid, tid = G.tid;
     TmaTile T, Tn;
@@ -210,7 +213,7 @@ __global__ void __launch_bounds__(FuShape<C, HW>::THREADS, 1) dct_fused_kernel(c
     using F = FuShape<C, HW>;
     using S = TmaShape<C>;
     extern __shared__ __align__(128) uint32_t smem[];
-    int *progress = reinterpret_cast<int *>(reinterpret_cast<uint8_t *>(smem) + T0_WORDS * 4 + FU_CTL_OFFSET);
+    int *progress = reinterpret_cast<int *>(reinterpret_cast<uint8_t *>(smem) + FU_TABLE_BYTES + FU_CTL_OFFSET);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // the tile warps come FIRST: the issue arbiter favours the CTA's oldest warps, and the tile warps, which are latency-bound and
     // ask for few issue slots, must never queue behind the always-ready hash warps (measured: placed last they were starved
@@ -219,11 +222,15 @@ __global__ void __launch_bounds__(FuShape<C, HW>::THREADS, 1) dct_fused_kernel(c
     const int gid = tile_wg ? warp / S::WARPS : 0, tid = tile_wg ? (warp % S::WARPS) * 32 + lane : 0;
     const bool tile_warp = tile_wg && gid < F::NP;             // (C = 3: two warps of the tile warpgroups have no group)
     if (tile_warp && tid == 0) {
-        const uint32_t bar = smem_u32(reinterpret_cast<uint8_t *>(smem) + T0_WORDS * 4 + 16 * gid);
+        const uint32_t bar = smem_u32(reinterpret_cast<uint8_t *>(smem) + FU_TABLE_BYTES + 16 * gid);
         mbar_init(bar, 1); mbar_init(bar + 8, 1); mbar_init_fence();
     }
     if (threadIdx.x < F::NP) progress[threadIdx.x] = 0;
-    load_t0_replicated(smem);   // ends with __syncthreads
+    {   // T0..T3, every entry replicated 32 times (lane l reads copy l in bank l)
+        const uint32_t *src = &g_aes.T[0][0];
+        for (int i = threadIdx.x; i < REP4_TABLE_WORDS; i += blockDim.x) smem[i] = src[i >> 5];
+        __syncthreads();
+    }
     const FuWork W = fu_work<C>(p);
     if (!tile_wg) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(FU_HASH_REGS));
@@ -231,10 +238,10 @@ __global__ void __launch_bounds__(FuShape<C, HW>::THREADS, 1) dct_fused_kernel(c
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F::TILE_REGS));
         if (tile_warp) {
-            const TmaGroup<C> G = tma_group_setup<C>(smem, p.k, gid, tid);
-            T0Lane sT;
-            sT.tab = reinterpret_cast<const char *>(smem);
-            sT.lane4 = 4u * lane;
+            const TmaGroup<C> G = tma_group_setup<C>(smem, p.k, gid, tid, FU_TABLE_BYTES);
+            RepAes sT;
+            sT.base = smem_u32(smem) + 4u * lane;
+            sT.c128 = p.c128;
             if (FRAGMENT) fu_fragment_tiles<C, V, F::NP, F::TPU>(p, W, sT, G, progress);
             else fu_defragment_tiles<C, V, F::NP, F::TPU>(p, W, sT, G);
         }

@@ -23,6 +23,7 @@
 // row segments are 16-byte multiples at 16-byte aligned addresses) and w / 8 >= TB (a tile spans at most two block rows).
 #pragma once
 #include "feds_dct_tile.cuh"
+#include "feds_aes_rep.cuh"
 
 namespace feds {
 
@@ -44,9 +45,13 @@ template <int C> __host__ __device__ inline int tma_stage_words(int k) {
     return C * (tile_run_stride(TmaShape<C>::TB * (63 - k)) + tile_run_stride(TmaShape<C>::TB * (k + 1)));
 }
 template <int C> __host__ __device__ inline size_t tma_group_bytes(int k) { return (size_t)2 * TmaShape<C>::PIX_BYTES + (size_t)tma_stage_words<C>(k) * 4; }
-template <int C> __host__ __device__ inline size_t tma_smem_bytes(int k, int groups) {
-    return (size_t)T0_WORDS * 4 + TMA_BAR_BYTES + (size_t)groups * tma_group_bytes<C>(k);
+// `table_bytes`: the AES tables in front of everything else (T0 32-fold: 32 KB; the four-table layout of feds_aes_rep.cuh: 128 KB)
+template <int C> __host__ __device__ inline size_t tma_smem_bytes(int k, int groups, size_t table_bytes = (size_t)T0_WORDS * 4) {
+    return table_bytes + TMA_BAR_BYTES + (size_t)groups * tma_group_bytes<C>(k);
 }
+// one AES block on whichever table layout the kernel holds
+template <bool SMALL, typename RkPtr> __device__ __forceinline__ void tile_aes(const T0Lane &T, const RkPtr rk, uint32_t (&s)[4]) { aes128_encrypt<SMALL>(T, rk, s); }
+template <bool SMALL, typename RkPtr> __device__ __forceinline__ void tile_aes(const RepAes &A, const RkPtr rk, uint32_t (&s)[4]) { aes128_encrypt_rep32<SMALL>(A, rk, s); }
 template <int C> __host__ __device__ inline bool tma_shape_ok(int w) { return (w % 32) == 0 && (w / 8) >= TmaShape<C>::TB; }
 
 // ------------------------------------------------------------------------------------------------------------ PTX wrappers
@@ -217,8 +222,8 @@ __device__ __forceinline__ void tma_block_dct(const uint8_t *s_pix, const TmaTil
 
 // AES-128-CTR over the staged private runs of a tile by the whole group (k + 1 not a multiple of 4): every counter block that
 // overlaps a run is computed once. Run c holds words [W0_c, W0_c + nb * P) of the image's private stream.
-template <int C, bool SMALL = false>
-__device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lane &sT, const TmaTile &T, uint32_t *s_priv, int RSP, int P, int tid) {
+template <int C, bool SMALL = false, typename Tab>
+__device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const Tab &sT, const TmaTile &T, uint32_t *s_priv, int RSP, int P, int tid) {
     constexpr int THREADS = TmaShape<C>::THREADS, TB = TmaShape<C>::TB;
     uint32_t nonce[4];
     load_nonce(p, T.n, nonce);
@@ -233,7 +238,7 @@ __device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lan
         if (first >= nw) continue;
         uint32_t ks[4];
         ctr_block(nonce, blk, ks);
-        aes128_encrypt<SMALL>(sT, p.rk, ks);
+        tile_aes<SMALL>(sT, p.rk, ks);
         uint32_t *run = s_priv + c * RSP;
         if (first >= 0 && first + 4 <= nw && (first & 3) == 0) {
             uint4 x = *reinterpret_cast<uint4 *>(run + first);
@@ -249,15 +254,15 @@ __device__ __forceinline__ void tma_aes_ctr_runs(const DctParams &p, const T0Lan
     }
 }
 // AES-128-CTR of one block's own private words in the stage (4 | k + 1: they are whole counter blocks)
-template <bool SMALL = false>
-__device__ __forceinline__ void tma_aes_ctr_own(const DctParams &p, const T0Lane &sT, int n, unsigned long long w0, int P, uint32_t *my_priv) {
+template <bool SMALL = false, typename Tab>
+__device__ __forceinline__ void tma_aes_ctr_own(const DctParams &p, const Tab &sT, int n, unsigned long long w0, int P, uint32_t *my_priv) {
     uint32_t nonce[4];
     load_nonce(p, n, nonce);
 #pragma unroll 1
     for (int g = 0; g < P; g += 4) {
         uint32_t ks[4];
         ctr_block(nonce, (w0 + g) >> 2, ks);
-        aes128_encrypt<SMALL>(sT, p.rk, ks);
+        tile_aes<SMALL>(sT, p.rk, ks);
         uint4 x = *reinterpret_cast<uint4 *>(my_priv + g);
         x.x ^= ks[0]; x.y ^= ks[1]; x.z ^= ks[2]; x.w ^= ks[3];
         *reinterpret_cast<uint4 *>(my_priv + g) = x;
@@ -273,18 +278,18 @@ template <int C> struct TmaGroup {
     uint32_t bar[2];              // mbarriers (shared addresses)
 };
 template <int C>
-__device__ __forceinline__ TmaGroup<C> tma_group_setup(uint32_t *smem, int k, int gid, int tid) {
+__device__ __forceinline__ TmaGroup<C> tma_group_setup(uint32_t *smem, int k, int gid, int tid, size_t table_bytes = (size_t)T0_WORDS * 4) {
     using S = TmaShape<C>;
     TmaGroup<C> G;
     G.gid = gid; G.tid = tid;
     const int warp = tid >> 5, lane = tid & 31;
     G.ch = warp % C; G.j = (warp / C) * 32 + lane;
-    uint8_t *base = reinterpret_cast<uint8_t *>(smem) + T0_WORDS * 4 + TMA_BAR_BYTES + (size_t)gid * tma_group_bytes<C>(k);
+    uint8_t *base = reinterpret_cast<uint8_t *>(smem) + table_bytes + TMA_BAR_BYTES + (size_t)gid * tma_group_bytes<C>(k);
     G.pix[0] = base; G.pix[1] = base + S::PIX_BYTES;
     G.RSQ = tile_run_stride(S::TB * (63 - k)); G.RSP = tile_run_stride(S::TB * (k + 1));
     G.s_pub = reinterpret_cast<uint32_t *>(base + 2 * S::PIX_BYTES);
     G.s_priv = G.s_pub + C * G.RSQ;
-    G.bar[0] = smem_u32(reinterpret_cast<uint8_t *>(smem) + T0_WORDS * 4 + 16 * gid);
+    G.bar[0] = smem_u32(reinterpret_cast<uint8_t *>(smem) + table_bytes + 16 * gid);
     G.bar[1] = G.bar[0] + 8;
     return G;
 }
@@ -293,8 +298,8 @@ __device__ __forceinline__ TmaGroup<C> tma_group_setup(uint32_t *smem, int k, in
 // One tile, from the pixel tile in shared memory (already waited for) to the stage: DCT, zigzag split, AES. Ends with the
 // barrier after which the elected thread may issue the bulk stores. `pre_stage` runs between the arithmetic and the first write
 // to the stage (the caller waits there until the previous tile's stores have read the stage).
-template <int C, int V, bool SMALL = false, typename PreStage>
-__device__ __forceinline__ void tma_fragment_tile(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, const uint8_t *s_pix,
+template <int C, int V, bool SMALL = false, typename Tab, typename PreStage>
+__device__ __forceinline__ void tma_fragment_tile(const DctParams &p, const Tab &sT, const TmaGroup<C> &G, const TmaTile &T, const uint8_t *s_pix,
                                                   PreStage &&pre_stage) {
     constexpr ZigzagTable ZZ = make_zigzag();
     constexpr int THREADS = TmaShape<C>::THREADS;
@@ -356,8 +361,8 @@ __global__ void __launch_bounds__(TmaShape<C>::CTA, 1) fragment_dct_tma_kernel(c
 
 // ------------------------------------------------------------------------------------------------------------ defragment: steps 6-8
 // stage (already waited for) -> decrypt, merge, IDCT -> packed rows of this thread's block in registers (2 words per row)
-template <int C, int V, bool SMALL = false>
-__device__ __forceinline__ void tma_defragment_block(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, uint32_t (&rows)[16]) {
+template <int C, int V, bool SMALL = false, typename Tab>
+__device__ __forceinline__ void tma_defragment_block(const DctParams &p, const Tab &sT, const TmaGroup<C> &G, const TmaTile &T, uint32_t (&rows)[16]) {
     constexpr ZigzagTable ZZ = make_zigzag();
     const int P = p.k + 1, Q = 63 - p.k;
     uint32_t *my_pub = G.s_pub + G.ch * G.RSQ + G.j * Q - P;   // indexed by z
@@ -414,8 +419,8 @@ __device__ __forceinline__ void tma_interleave(const TmaTile &T, const uint8_t *
 // One tile from the stage (already waited for) to the out tile in shared memory, ending with the barrier after which the elected
 // thread may issue the pixel stores. `stage_read` runs right after the barrier that follows the last read of the stage (the caller
 // refills the stage there); before that barrier the elected thread has waited for the previous out tile to be read.
-template <int C, int V, bool SMALL = false, typename StageRead>
-__device__ __forceinline__ void tma_defragment_tile(const DctParams &p, const T0Lane &sT, const TmaGroup<C> &G, const TmaTile &T, StageRead &&stage_read) {
+template <int C, int V, bool SMALL = false, typename Tab, typename StageRead>
+__device__ __forceinline__ void tma_defragment_tile(const DctParams &p, const Tab &sT, const TmaGroup<C> &G, const TmaTile &T, StageRead &&stage_read) {
     constexpr int THREADS = TmaShape<C>::THREADS, TB = TmaShape<C>::TB;
     const bool act = G.j < T.nb;
     if (V != 4) {
