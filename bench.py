@@ -579,6 +579,25 @@ def main():
             e1.record()
             torch.cuda.synchronize()
             return e0.elapsed_time(e1) / reps
+        # the same path on a batch of 4 such images (feds_*_dwt_batch): one image is a single half-empty wave of leaf-hash chains,
+        # a batch fills the machine -- per-image time and the leaf-hash kernel's ALU fraction are what changes
+        nb_ = 4
+        db = B.DwtBatch(nb_, w, h, c, kl, device=dev)
+        b_in = d_img.unsqueeze(0).repeat(nb_, 1, 1, 1).contiguous()
+        b_out = torch.empty_like(b_in)
+        b_non = torch.from_numpy(sharding.nonces_for(nonce, 0, nb_, priv_bytes=db.priv_bytes)).to(dev)
+        e_a, e_b = ev(), ev()
+        B.profile_events(e_a, e_b)
+        bf = timed_dwt(lambda: db.fragment(b_in, key, b_non))
+        B.profile_events(None, None)
+        torch.cuda.synchronize()
+        leaf4 = e_a.elapsed_time(e_b)
+        bd = timed_dwt(lambda: db.defragment(b_out, key, b_non, expected=db.digests))
+        assert torch.equal(b_out, b_in) and int(db.flags_out.abs().sum().item()) == 0
+        stages["batch_of_4"] = {"fragment_ms_per_image": bf / nb_, "defragment_verify_ms_per_image": bd / nb_,
+                                "MBps": nb_ * step_image_bytes / ((bf + bd) * 1e-3) / 1e6, "leaf_hash_kernel_ms": leaf4,
+                                "leaf_hash_alu_frac": nb_ * alu_ops / (leaf4 * 1e-3) / 1e12 / alu_peak}
+        del db, b_in, b_out
         tb = B.TilesBatch(1, w, h, c, device=dev)
         t_non = torch.from_numpy(np.frombuffer(nonce, dtype=np.uint8).copy()).to(dev).view(1, 16)
         t_in, t_out = d_img.unsqueeze(0).contiguous(), torch.empty_like(d_img).unsqueeze(0)
