@@ -57,12 +57,14 @@ int tree_levels(unsigned leaves, unsigned n[40]) {
     while (n[L - 1] > 1) { n[L] = (n[L - 1] + FANOUT - 1) / FANOUT; ++L; }
     return L;
 }
-// bytes of digest storage for one tree, all levels with more than one node (the single-node level is the root)
+// bytes of digest storage for one tree, all levels with more than one node (the single-node level is the root), and the
+// arrival counters of the spread-out tree top
 size_t tree_bytes(unsigned leaves) {
     unsigned n[40];
     const int L = tree_levels(leaves, n);
     size_t b = 0;
     for (int i = 0; i < L; ++i) if (n[i] > 1) b += (size_t)n[i] * 32;
+    if (leaves > 1) b += TOP_CTRL_BYTES;   // arrival counters of merkle_top_kernel
     return b;
 }
 

@@ -28,6 +28,10 @@ struct MerkleLevelParams {
     uint8_t *out2;
     unsigned n_in2, n_trees2;
     size_t in2_tree_stride, out2_tree_stride;
+    // merkle_top_kernel only: global scratch for the two levels under the root of each family ([tree][node][32] per level, the
+    // level of <= 256 nodes first) and TOP_CTRL_WORDS zeroed arrival counters per tree (trees of family 2 after those of family 1)
+    uint8_t *scratch, *scratch2;
+    unsigned *ctrl;
 };
 
 // SHA-256 of `cnt` (1..16) concatenated 32-byte child digests at src (global memory via the read-only path, or shared).
@@ -132,6 +136,67 @@ __global__ void __launch_bounds__(TAIL_THREADS) merkle_tail_kernel(const __grid_
         __syncthreads();
         src = dst; dst = (dst == sA) ? sB : sA; n = m;
     }
+}
+
+// The same top of a tree spread over the chip, for calls with only a few trees (a single image): merkle_tail_kernel walks three
+// levels on ONE SM -- 18 + 18 + 13 us of dependent compressions for the 4096 -> 256 -> 16 -> 1 top of a 134 MB stream. Here every
+// node of every level is hashed by a cooperating warp (sha256_warp_coop, ~13 us for the nine blocks of a 16-child node: a lone
+// warp sustains one round per ~45 cycles) and a CTA holds only four of them, one per warp scheduler: CTA c of a tree hashes nodes
+// 4c .. 4c+3 of the first level into global scratch; the LAST of the (up to four) CTAs under one second-level node to finish -- an
+// arrival counter per node, the threadfence + atomic ticket pattern -- hashes that node with its warp 0, and the last of those
+// hashes the root. Three levels in 3 x 13 us (measured 44 us against 56), no grid-wide barrier, counters zeroed by a memset node in
+// front of the launch.
+constexpr int TOP_WARPS = 4, TOP_THREADS = TOP_WARPS * 32, TOP_CTRL_WORDS = 32, TOP_MAX_TREES = 8;   // TOP_CTRL_BYTES (feds_host.h) covers two trees
+constexpr unsigned TOP_CTAS_PER_TREE = 256 / TOP_WARPS;
+__global__ void __launch_bounds__(TOP_THREADS) merkle_top_kernel(const __grid_constant__ MerkleLevelParams p) {
+    __shared__ __align__(16) uint32_t s_ws[TOP_WARPS * coop_ws_words<TAIL_STRIDE>()];
+    __shared__ __align__(16) uint4 s_kids[2 * FANOUT];
+    __shared__ unsigned s_ticket;
+    const unsigned t = blockIdx.y, c = blockIdx.x, tid = threadIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool extra = t >= p.n_trees;
+    if (!extra && p.odd_trees_only_if_nonempty && (t & 1u)) return;
+    const unsigned t2 = extra ? t - p.n_trees : t;
+    const unsigned n = extra ? p.n_in2 : p.n_in, m1 = (n + FANOUT - 1) / FANOUT, m2 = (m1 + FANOUT - 1) / FANOUT;
+    if (c * TOP_WARPS >= m1) return;
+    const unsigned trees = extra ? p.n_trees2 : p.n_trees;
+    const uint8_t *src = extra ? p.in2 + (size_t)t2 * p.in2_tree_stride : p.in + (size_t)t2 * p.in_tree_stride;
+    uint8_t *root = extra ? p.out2 + (size_t)t2 * p.out2_tree_stride : p.out + (size_t)t2 * p.out_tree_stride;
+    uint8_t *sc = extra ? p.scratch2 : p.scratch;
+    uint8_t *lvA = sc + (size_t)t2 * m1 * 32, *lvB = sc + (size_t)trees * m1 * 32 + (size_t)t2 * m2 * 32;
+    unsigned *ctrl = p.ctrl + (size_t)t * TOP_CTRL_WORDS;
+    uint32_t *ws = s_ws + warp * coop_ws_words<TAIL_STRIDE>();
+    uint32_t H[8];
+    const unsigned a = c * TOP_WARPS + warp;
+    if (a < m1) {
+        const unsigned lo = a * FANOUT, cnt = min(lo + FANOUT, n) - lo;
+        sha256_warp_coop<TAIL_STRIDE>(src + (size_t)lo * 32, cnt * 32u, ws, (int)lane, p.one, H);
+        if (lane == 0) { store_digest(m1 == 1 ? root : lvA + (size_t)a * 32, H); __threadfence(); }
+    }
+    if (m1 == 1) return;
+    const unsigned b = c * TOP_WARPS / FANOUT;   // second-level node over this CTA's four nodes
+    const unsigned kids = min(b * FANOUT + FANOUT, m1) - b * FANOUT;
+    __syncthreads();
+    if (tid == 0) { __threadfence(); s_ticket = atomicAdd(&ctrl[b], 1u); }
+    __syncthreads();
+    if (s_ticket != (kids + TOP_WARPS - 1) / TOP_WARPS - 1 || warp != 0) return;
+    __threadfence();
+    if (lane < 2 * kids) s_kids[lane] = __ldcg(reinterpret_cast<const uint4 *>(lvA + (size_t)b * FANOUT * 32) + lane);
+    __syncwarp();
+    sha256_warp_coop<TAIL_STRIDE>(reinterpret_cast<const uint8_t *>(s_kids), kids * 32u, ws, (int)lane, p.one, H);
+    unsigned ticket = 0;
+    if (lane == 0) {
+        store_digest(m2 == 1 ? root : lvB + (size_t)b * 32, H);
+        if (m2 > 1) { __threadfence(); ticket = atomicAdd(&ctrl[FANOUT], 1u); }
+    }
+    if (m2 == 1) return;
+    ticket = __shfl_sync(0xffffffffu, ticket, 0);
+    if (ticket != m2 - 1) return;
+    __threadfence();
+    __syncwarp();
+    if (lane < 2 * m2) s_kids[lane] = __ldcg(reinterpret_cast<const uint4 *>(lvB) + lane);
+    __syncwarp();
+    sha256_warp_coop<TAIL_STRIDE>(reinterpret_cast<const uint8_t *>(s_kids), m2 * 32u, ws, (int)lane, p.one, H);
+    if (lane == 0) store_digest(root, H);
 }
 
 // ------------------------------------------------------------------------------------------------------------

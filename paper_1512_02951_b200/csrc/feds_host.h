@@ -68,6 +68,8 @@ feds_status launch_packed_private_leaves(const DctParams &p, int c, cudaStream_t
 feds_status launch_fragment_dwt_tiles(const DctParams &p, int c, cudaStream_t stream);
 feds_status launch_defragment_dwt_tiles(const DctParams &p, int c, cudaStream_t stream);
 // ---- feds_k_hash.cu: Merkle upper levels, stream leaves, AES-CTR stream, digest compare
+// Every tree's scratch (all levels with more than one node above level 0) ends with TOP_CTRL_BYTES for merkle_top_kernel's counters.
+constexpr size_t TOP_CTRL_BYTES = 256;
 feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8_t *scratch, uint8_t *roots, size_t root_stride,
                      int skip_odd, cudaStream_t stream);
 feds_status run_two_trees(const uint8_t *l0a, unsigned na, uint8_t *sca, uint8_t *roota, const uint8_t *l0b, unsigned nb, uint8_t *scb,

@@ -20,6 +20,26 @@ feds_status tail_smem_once() {
     return set_smem_once(merkle_tail_kernel, TAIL_SMEM_BYTES, smem_set);
 }
 
+// the top of a few trees spread over the chip (merkle_top_kernel): pays when merkle_tail_kernel would hash TWO levels one node per
+// thread, i.e. more than 64 nodes in the first (measured: 8192^2 DWT, 256 nodes, 56 -> 44 us; 512^2 DCT, 32 nodes, 33 -> 37 + the
+// memset). `spare` = the end of the primary family's level storage (tree_bytes keeps TOP_CTRL_BYTES per tree)
+bool top_pays(unsigned total_trees, unsigned na, unsigned nb) {
+    const unsigned ma = (na + FANOUT - 1) / FANOUT, mb = (nb + FANOUT - 1) / FANOUT;
+    return total_trees <= (unsigned)TOP_MAX_TREES && std::max(ma, mb) > 4u * FANOUT;
+}
+size_t top_levels_bytes(unsigned n, unsigned n_trees) {
+    const unsigned m1 = (n + FANOUT - 1) / FANOUT, m2 = (m1 + FANOUT - 1) / FANOUT;
+    return (size_t)n_trees * ((m1 > 1 ? m1 : 0) + (m2 > 1 ? m2 : 0)) * 32;
+}
+feds_status launch_top(MerkleLevelParams &mp, unsigned total_trees, uint8_t *spare, cudaStream_t stream) {
+    static_assert(TOP_CTRL_BYTES >= 2 * TOP_CTRL_WORDS * 4, "the primary family's spare bytes hold the counters of both families");
+    mp.ctrl = reinterpret_cast<unsigned *>(spare);
+    FEDS_CUDA(cudaMemsetAsync(spare, 0, (size_t)total_trees * TOP_CTRL_WORDS * 4, stream));
+    merkle_top_kernel<<<dim3(TOP_CTAS_PER_TREE, total_trees), TOP_THREADS, 0, stream>>>(mp);
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+
 // wide levels of n_trees equal trees: one thread per node until at most TAIL_MAX_IN digests per tree remain
 feds_status reduce_wide(const uint8_t *&in, unsigned &n, unsigned n_trees, uint8_t *&sc, int skip_odd, cudaStream_t stream) {
     MerkleLevelParams mp{};
@@ -55,6 +75,10 @@ feds_status run_tree(const uint8_t *level0, unsigned n0, unsigned n_trees, uint8
         mp.n_trees = n_trees; mp.odd_trees_only_if_nonempty = skip_odd; mp.one = 1u;
         mp.in = in; mp.n_in = n; mp.n_out = 1; mp.in_tree_stride = (size_t)n * 32;
         mp.out = roots; mp.out_tree_stride = root_stride;
+        if (top_pays(n_trees, n, 0)) {
+            mp.scratch = sc;
+            return launch_top(mp, n_trees, sc + top_levels_bytes(n, n_trees), stream);
+        }
         feds_status ts = tail_smem_once();
         if (ts != FEDS_OK) return ts;
         merkle_tail_kernel<<<n_trees, TAIL_THREADS, TAIL_SMEM_BYTES, stream>>>(mp);
@@ -76,18 +100,23 @@ feds_status run_two_trees(const uint8_t *l0a, unsigned na, uint8_t *sca, uint8_t
     MerkleLevelParams mp{};
     mp.one = 1u; mp.n_out = 1;
     unsigned ctas = 0;
+    uint8_t *spare = nullptr;
     if (na > 1) {
         mp.n_trees = n_trees; mp.in = ina; mp.n_in = na; mp.in_tree_stride = (size_t)na * 32; mp.out = roota; mp.out_tree_stride = root_stride;
+        mp.scratch = sca; spare = sca + top_levels_bytes(na, n_trees);
         ctas = n_trees;
     }
     if (nb > 1) {
         if (ctas == 0) {
             mp.n_trees = n_trees; mp.in = inb; mp.n_in = nb; mp.in_tree_stride = (size_t)nb * 32; mp.out = rootb; mp.out_tree_stride = root_stride;
+            mp.scratch = scb; spare = scb + top_levels_bytes(nb, n_trees);
         } else {
             mp.in2 = inb; mp.n_in2 = nb; mp.n_trees2 = n_trees; mp.in2_tree_stride = (size_t)nb * 32; mp.out2 = rootb; mp.out2_tree_stride = root_stride;
+            mp.scratch2 = scb;
         }
         ctas += n_trees;
     }
+    if (top_pays(ctas, na > 1 ? na : 0, nb > 1 ? nb : 0)) return launch_top(mp, ctas, spare, stream);
     feds_status ts = tail_smem_once();
     if (ts != FEDS_OK) return ts;
     merkle_tail_kernel<<<ctas, TAIL_THREADS, TAIL_SMEM_BYTES, stream>>>(mp);

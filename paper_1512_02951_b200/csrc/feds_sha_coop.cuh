@@ -8,7 +8,7 @@
 //   phase 2: the rounds of those blocks run one after the other (every lane computes the same values: no divergence, broadcast
 //            loads), each round a chain of three dependent instructions: e' = (d + h + K_t + W_t) + Sigma1(e) + Ch(e, f, g)
 //            with the bracket formed off the critical path.
-// ~900 cycles per block instead of ~3,900. Throughput is a 32nd of a thread-per-message kernel's, so the host uses these kernels
+// ~2,900 cycles per block instead of ~3,900 (a lone warp cannot issue the ~16 instructions of a round in less than ~45 cycles). Throughput is a 32nd of a thread-per-message kernel's, so the host uses these kernels
 // only while there are fewer messages than the chip has warp schedulers to spare (small images, tree tops).
 #pragma once
 #include "feds_device.cuh"

@@ -57,7 +57,9 @@ def test_aes_ctr_sp800_38a_f51(orc, b, kat):
 
 
 # leaves: none, one short, exactly one, one + 1 byte, 16 leaves (one node), 17, 4096 (tail kernel limit), 4097 (a wide level), big ragged
-@pytest.mark.parametrize("n", [0, 5, 2048, 2049, 16 * 2048, 17 * 2048 - 3, 4096 * 2048, 4097 * 2048 + 11, 30_000_001])
+# the last four: tree tops of 65 / 65 / 128 / 252 first-level nodes, ragged at every level (the spread-out top kernel's counters)
+@pytest.mark.parametrize("n", [0, 5, 2048, 2049, 16 * 2048, 17 * 2048 - 3, 4096 * 2048, 4097 * 2048 + 11, 30_000_001,
+                               1024 * 2048 + 1, 1030 * 2048 + 5, 2047 * 2048 + 1, 4032 * 2048 - 7])
 def test_sha256_merkle_matches_oracle(orc, b, n):
     data = _bytes(n, n + 1)
     root = b.sha256_merkle(torch.from_numpy(data).cuda())
