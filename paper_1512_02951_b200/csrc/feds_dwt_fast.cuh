@@ -77,22 +77,45 @@ __device__ __forceinline__ void store_i16(int16_t *dst, const int (&v)[N]) {
 template <int C, int PX, bool U8>
 struct FwdRow {
     static constexpr int NV = PX * C, HP = PX / 2;
-    // loads image / plane row y for the lane's run starting at pixel px0 and lifts it horizontally
-    static __device__ __forceinline__ void get(const DwtLevelParams &p, const void *base, int y, int px0, bool in_range, bool first_run,
-                                               bool last_run, int (&lo)[HP * C], int (&hi)[HP * C]) {
-        int v[NV];
+    static constexpr int RAW = U8 ? NV / 4 : NV / 2;   // 32-bit words of one row of this lane's run as loaded
+    // image / plane row y of the lane's run starting at pixel px0, as loaded (the loop keeps the next two rows in flight)
+    static __device__ __forceinline__ void load(const DwtLevelParams &p, const void *base, int y, int px0, bool in_range, uint32_t (&w)[RAW]) {
         if (in_range) {
             if (U8) {
-                uint32_t w[NV / 4];
-                load_bytes<NV>(static_cast<const uint8_t *>(base) + ((size_t)y * p.img_w + px0) * C, w);
-#pragma unroll
-                for (int i = 0; i < NV; ++i) v[i] = (int)((w[i >> 2] >> (8 * (i & 3))) & 0xffu) - 128;
+                load_bytes<NV>(static_cast<const uint8_t *>(base) + ((size_t)y * p.img_w + px0) * C, reinterpret_cast<uint32_t(&)[NV / 4]>(w));
             } else {
-                load_i16<NV>(static_cast<const int16_t *>(base) + (size_t)y * p.cw + px0, v);
+                const uint4 *src = reinterpret_cast<const uint4 *>(static_cast<const int16_t *>(base) + (size_t)y * p.cw + px0);
+                if (NV == 4) {
+                    const uint2 q = __ldg(reinterpret_cast<const uint2 *>(src));
+                    w[0] = q.x; w[1 % RAW] = q.y;
+                } else {
+#pragma unroll
+                    for (int i = 0; i < NV / 8; ++i) {
+                        const uint4 q = __ldg(src + i);
+                        w[(4 * i) % RAW] = q.x; w[(4 * i + 1) % RAW] = q.y; w[(4 * i + 2) % RAW] = q.z; w[(4 * i + 3) % RAW] = q.w;
+                    }
+                }
             }
         } else {
 #pragma unroll
-            for (int i = 0; i < NV; ++i) v[i] = 0;
+            for (int i = 0; i < RAW; ++i) w[i] = U8 ? 0x80808080u : 0u;   // lifts to zeros
+        }
+    }
+    static __device__ __forceinline__ void get(const DwtLevelParams &p, const void *base, int y, int px0, bool in_range, bool first_run,
+                                               bool last_run, int (&lo)[HP * C], int (&hi)[HP * C]) {
+        uint32_t w[RAW];
+        load(p, base, y, px0, in_range, w);
+        lift(w, first_run, last_run, lo, hi);
+    }
+    // horizontal lifting of a loaded row
+    static __device__ __forceinline__ void lift(const uint32_t (&w)[RAW], bool first_run, bool last_run, int (&lo)[HP * C], int (&hi)[HP * C]) {
+        int v[NV];
+        if (U8) {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) v[i] = (int)((w[i >> 2] >> (8 * (i & 3))) & 0xffu) - 128;
+        } else {
+#pragma unroll
+            for (int i = 0; i < NV / 2; ++i) { v[2 * i] = (int)(int16_t)(w[i % RAW] & 0xffffu); v[2 * i + 1] = (int)w[i % RAW] >> 16; }
         }
         int rn[C];  // x[PX] of this run = the right neighbour's first pixel; x[cw] = x[cw-2] at the image border
 #pragma unroll
@@ -157,16 +180,26 @@ __global__ void __launch_bounds__(DWTF_WARPS * 32) dwt_fwd_fast_kernel(const __g
 #pragma unroll
         for (int i = 0; i < NH; ++i) { Plo[i] = 0; Phi[i] = 0; }
     }
+    uint32_t rO[Row::RAW], rN[Row::RAW];   // rows 2m+1 and 2m+2 as loaded, one iteration ahead of their use (two ahead gained nothing)
+    Row::load(p, base, 2 * m0 + 1, px0, in_range, rO);
+    Row::load(p, base, min(2 * m0 + 2, p.ch - 1), px0, in_range, rN);
 #pragma unroll 1
     for (int m = m0; m < m1; ++m) {
+        uint32_t nO[Row::RAW], nN[Row::RAW];
+        if (m + 1 < m1) {
+            Row::load(p, base, 2 * m + 3, px0, in_range, nO);
+            Row::load(p, base, min(2 * m + 4, p.ch - 1), px0, in_range, nN);
+        }
         int Olo[NH], Ohi[NH], Nlo[NH], Nhi[NH];
-        Row::get(p, base, 2 * m + 1, px0, in_range, first_run, last_run, Olo, Ohi);
+        Row::lift(rO, first_run, last_run, Olo, Ohi);
         if (2 * m + 2 < p.ch) {
-            Row::get(p, base, 2 * m + 2, px0, in_range, first_run, last_run, Nlo, Nhi);
+            Row::lift(rN, first_run, last_run, Nlo, Nhi);
         } else {  // h[ch] = h[ch-2]
 #pragma unroll
             for (int i = 0; i < NH; ++i) { Nlo[i] = Elo[i]; Nhi[i] = Ehi[i]; }
         }
+#pragma unroll
+        for (int i = 0; i < Row::RAW; ++i) { rO[i] = nO[i]; rN[i] = nN[i]; }
         int Slo[NH], Shi[NH];
 #pragma unroll
         for (int i = 0; i < NH; ++i) {
