@@ -1,6 +1,8 @@
 // feds_k_dct_strong.cu — launchers of the strong-level kernels (feds_dct_strong.cuh; PAPER.md 6.3.2) and of the packed-storage kernels
 // (feds_dct_packed.cuh; PAPER.md 6.4.3), which share the fixed-point basis table.
-#include "feds_dct_packed.cuh"
+#include <algorithm>
+
+#include "feds_dct_packed_tile.cuh"
 #include "feds_host.h"
 
 namespace feds {
@@ -38,8 +40,38 @@ feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t str
     return FEDS_OK;
 }
 
-// ---- packed integer storage: one thread per (leaf group, channel)
+// ---- packed integer storage: bulk-copy tile groups (feds_dct_packed_tile.cuh) where the shape allows, else one thread per
+// (leaf group, channel)
+namespace {
+template <int C, typename Kernel, typename... Extra>
+feds_status launch_packed_tile(Kernel kernel, size_t &smem_set, const DctParams &p, cudaStream_t stream, bool profile, Extra... extra) {
+    using S = TmaShape<C>;
+    using PS = PackedTileShape<C>;
+    const size_t smem = packed_tile_smem_bytes<C>();
+    feds_status s = set_smem_once(kernel, smem, smem_set);
+    if (s != FEDS_OK) return s;
+    const unsigned long long tiles = (unsigned long long)p.n_images * (((unsigned long long)p.nbr * p.nbc + S::TB - 1) / S::TB);
+    const unsigned grid = (unsigned)std::min<unsigned long long>((tiles + PS::GROUPS - 1) / PS::GROUPS, (unsigned long long)sm_count());
+    if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
+    kernel<<<grid, PS::CTA, smem, stream>>>(p, extra...);
+    if (prof_stop_event() && profile) FEDS_CUDA(cudaEventRecord(prof_stop_event(), stream));
+    FEDS_LAUNCH_CHECK();
+    return FEDS_OK;
+}
+bool packed_tile_supported(const DctParams &p, int c) {
+    if (p.generic_tiles) return false;
+    return c == 1 ? packed_tile_ok<1>(p.w, p.k) : c == 3 ? packed_tile_ok<3>(p.w, p.k) : packed_tile_ok<4>(p.w, p.k);
+}
+}  // namespace
+
 feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t stream, bool profile) {
+    if (packed_tile_supported(p, c)) {
+#define FEDS_PT(CC, PM) { static size_t set = 0; return launch_packed_tile<CC>(fragment_dct_packed_tile_kernel<CC, PM>, set, p, stream, profile); }
+#define FEDS_PT_P(CC) { if (p.k < 4) FEDS_PT(CC, 4) else if (p.k < 8) FEDS_PT(CC, 8) else FEDS_PT(CC, 16) }
+        if (c == 1) FEDS_PT_P(1) else if (c == 3) FEDS_PT_P(3) else FEDS_PT_P(4)
+#undef FEDS_PT_P
+#undef FEDS_PT
+    }
     const unsigned long long threads = (unsigned long long)p.n_images * c * p.nbr * p.nlr;
     const unsigned grid = (unsigned)((threads + PACKED_THREADS - 1) / PACKED_THREADS);
     const size_t smem = (size_t)64 * PACKED_THREADS * 4;
