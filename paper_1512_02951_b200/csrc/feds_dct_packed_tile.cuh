@@ -81,6 +81,25 @@ __device__ __forceinline__ void packed_remainder_words(const uint32_t (&x)[16], 
         r[i] = __byte_perm(__byte_perm((uint32_t)acc[4 * i], (uint32_t)acc[4 * i + 1], 0x0062u), __byte_perm((uint32_t)acc[4 * i + 2], (uint32_t)acc[4 * i + 3], 0x0062u), 0x5410u);
 }
 
+// The inverse: x = pub + floor((S + 2^11) / 2^12) mod 256 = byte 2 of (pub << 16 | 0x8000) + sum (16 q_z) B_z. q16[z] = 16 q_z.
+template <int HALF, int PMAX>
+__device__ __forceinline__ void packed_restore_words(const uint32_t (&x)[16], const int32_t (&q16)[PMAX], int P, uint32_t (&r)[8]) {
+    int32_t acc[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) acc[i] = (int32_t)__byte_perm(x[8 * HALF + (i >> 2)], 0x00008000u, 0x7054u + ((uint32_t)(i & 3) << 8));
+#pragma unroll
+    for (int z = 0; z < PMAX; ++z) {
+        if (z < P) {   // warp-uniform
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                acc[i] = (int32_t)((uint32_t)acc[i] + (uint32_t)q16[z] * (uint32_t)c_strong_basis_tab.B[64 * z + 32 * HALF + i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        r[i] = __byte_perm(__byte_perm((uint32_t)acc[4 * i], (uint32_t)acc[4 * i + 1], 0x0062u), __byte_perm((uint32_t)acc[4 * i + 2], (uint32_t)acc[4 * i + 3], 0x0062u), 0x5410u);
+}
+
 // ------------------------------------------------------------------------------------------------------------ fragment
 // the 64 bytes of block (j, ch) of the pixel tile, row-major, 16 words. Only this gather depends on the channel (immediate byte
 // selectors); everything after it is one copy of code for all warps.
@@ -196,6 +215,108 @@ __global__ void __launch_bounds__(PackedTileShape<C>::CTA, 1) fragment_dct_packe
         }
         group_sync(gid, S::THREADS);
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------ defragment
+// Shared memory per group as in the fragment kernel, used differently: [0] planar rows of the finished blocks, [1] the interleaved
+// out tile the bulk stores read (feds_dct_tma.cuh's defragment). `plain` = the decrypted private fragments (workspace).
+template <int C, int PMAX>
+__global__ void __launch_bounds__(PackedTileShape<C>::CTA, 1) defragment_dct_packed_tile_kernel(const __grid_constant__ DctParams p, const uint8_t *plain,
+                                                                                                size_t plain_stride) {
+    using S = TmaShape<C>;
+    using PS = PackedTileShape<C>;
+    constexpr int TB = S::TB;
+    extern __shared__ __align__(128) uint32_t smem[];
+    const int gid = threadIdx.x / S::THREADS, tid = threadIdx.x % S::THREADS, lane = threadIdx.x & 31;
+    const int ch = (tid >> 5) % C, j = ((tid >> 5) / C) * 32 + lane;
+    uint8_t *base = reinterpret_cast<uint8_t *>(smem) + TMA_BAR_BYTES;
+    uint8_t *planar = base + (size_t)gid * 2 * S::PIX_BYTES, *out_tile = planar + S::PIX_BYTES;
+    uint32_t *region = reinterpret_cast<uint32_t *>(base + (size_t)PS::GROUPS * 2 * S::PIX_BYTES) + (threadIdx.x >> 5) * PT_MAX_B;
+    const int b = (int)p.packed_group_bytes, P = p.k + 1, bits = p.ac_bits;
+    const unsigned tiles_per_plane = ((unsigned)p.nbr * p.nbc + TB - 1) / TB;
+    const unsigned total = (unsigned)p.n_images * tiles_per_plane, step = gridDim.x * PS::GROUPS;
+    const size_t plane = (size_t)p.nbr * p.nbc;
+    unsigned t = blockIdx.x * PS::GROUPS + gid;
+    // the block's 64 public bytes, one tile ahead
+    uint4 xn[4];
+    auto load_pub = [&](unsigned tt, uint4 (&x)[4]) {
+        const TmaTile T = tma_decode_tile<C>(p, tt, tiles_per_plane);
+        if (j < T.nb) {
+            const uint4 *src = reinterpret_cast<const uint4 *>(p.pub + (size_t)T.n * p.pub_stride + 64 * ((size_t)ch * plane + T.B0 + j));
+#pragma unroll
+            for (int i = 0; i < 4; ++i) x[i] = __ldg(src + i);
+        }
+    };
+    if (t < total) load_pub(t, xn);
+#pragma unroll 1
+    for (; t < total; t += step) {
+        const TmaTile T = tma_decode_tile<C>(p, t, tiles_per_plane);
+        const size_t blk0 = (size_t)ch * plane + T.B0;
+        const int j0 = j - lane, ngroups = min(4, (T.nb - j0) / 8);
+        if (ngroups > 0) {   // the warp's groups: ngroups * b bytes of the decrypted stream
+            const uint8_t *in = plain + (size_t)T.n * plain_stride + ((blk0 + j0) >> 3) * (size_t)b;
+            const int nbytes = ngroups * b;
+            if ((reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (nbytes & 3) == 0) {
+                for (int i = lane; i < (nbytes >> 2); i += 32) region[i] = __ldg(reinterpret_cast<const uint32_t *>(in) + i);
+            } else {
+                uint8_t *rb = reinterpret_cast<uint8_t *>(region);
+                for (int i = lane; i < nbytes; i += 32) rb[i] = __ldg(in + i);
+            }
+        }
+        uint32_t x[16];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { x[4 * i] = xn[i].x; x[4 * i + 1] = xn[i].y; x[4 * i + 2] = xn[i].z; x[4 * i + 3] = xn[i].w; }
+        if (t + step < total) load_pub(t + step, xn);
+        __syncwarp();
+        uint32_t rows[16];
+        if (j < T.nb) {
+            int32_t q[PMAX];
+            const unsigned bitpos = (unsigned)lane * (unsigned)b;
+            const uint32_t *word = region + (bitpos >> 5);
+            unsigned long long buf = (unsigned long long)(*word >> (bitpos & 31u));
+            int nbuf = 32 - (int)(bitpos & 31u);
+#pragma unroll
+            for (int z = 0; z < PMAX; ++z) {
+                q[z] = 0;
+                if (z < P) {
+                    const int nb = z == 0 ? 11 : bits;
+                    if (nbuf < nb) { buf |= (unsigned long long)*++word << nbuf; nbuf += 32; }
+                    const uint32_t field = (uint32_t)buf & ((1u << nb) - 1u);
+                    buf >>= nb;
+                    nbuf -= nb;
+                    int32_t v = (int32_t)field;
+                    if (z > 0) {
+                        const int32_t mag = (int32_t)(field & ((1u << (bits - 1)) - 1u));
+                        v = (field >> (bits - 1)) ? -mag : mag;
+                    }
+                    q[z] = 16 * v;
+                }
+            }
+            packed_restore_words<0, PMAX>(x, q, P, reinterpret_cast<uint32_t(&)[8]>(rows[0]));
+            packed_restore_words<1, PMAX>(x, q, P, reinterpret_cast<uint32_t(&)[8]>(rows[8]));
+        }
+        if (tid == 0) bulk_wait_read0();   // the previous tile's pixel stores have read the out tile
+        group_sync(gid, S::THREADS);
+        if constexpr (C == 1) {
+            if (j < T.nb) {
+                uint32_t off, pitch;
+                tma_pixel_slot<C>(T, j, off, pitch);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) *reinterpret_cast<uint2 *>(out_tile + off + r * pitch) = make_uint2(rows[2 * r], rows[2 * r + 1]);
+            }
+        } else {
+            if (j < T.nb) {
+#pragma unroll
+                for (int r = 0; r < 8; ++r) *reinterpret_cast<uint2 *>(planar + (ch * 8 + r) * (TB * 8) + j * 8) = make_uint2(rows[2 * r], rows[2 * r + 1]);
+            }
+            group_sync(gid, S::THREADS);
+            tma_interleave<C>(T, planar, out_tile, tid);
+        }
+        fence_proxy_async();
+        group_sync(gid, S::THREADS);
+        if (tid == 0) tma_move_pixels<C, true>(p, T, smem_u32(out_tile), 0u);
+    }
+    if (tid == 0) bulk_wait0();
 }
 
 }  // namespace feds

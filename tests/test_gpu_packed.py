@@ -74,7 +74,10 @@ def check(orc, b, img, k, bits, seed):
 
 @pytest.mark.parametrize("bits", [11, 8])
 @pytest.mark.parametrize("w,h,c,k", [(8, 8, 1, 0), (8, 8, 1, 5), (16, 16, 4, 63), (64, 8, 1, 3), (72, 24, 1, 5), (1080, 16, 3, 5), (136, 40, 4, 9),
-                                     (512, 512, 1, 5), (256, 264, 3, 5), (520, 24, 3, 26), (64, 64, 1, 32), (40, 8, 3, 4), (1920, 136, 3, 5)])
+                                     (512, 512, 1, 5), (256, 264, 3, 5), (520, 24, 3, 26), (64, 64, 1, 32), (40, 8, 3, 4), (1920, 136, 3, 5),
+                                     # w % 64 == 0 and a tile per block row: the bulk-copy tile kernels, all three PMAX forms, ragged last tiles
+                                     (256, 40, 4, 9), (320, 24, 3, 3), (512, 16, 1, 15), (256, 16, 3, 0), (576, 72, 4, 2), (1024, 24, 1, 7),
+                                     (512, 8, 1, 16), (1920, 8, 3, 12)])
 def test_packed_parity_and_round_trips(orc, b, w, h, c, k, bits):
     check(orc, b, synth.image(w, h, c, seed=w + 3 * h + c + k, rectangles=2 if w >= 64 and h >= 16 else 0), k, bits, seed=w * 3 + k + bits)
 
@@ -98,8 +101,9 @@ def test_packed_verify_flags(orc, b):
     assert int(fl.item()) == 1 and not torch.equal(rec, d_img)
 
 
-def test_packed_batch_equals_singles(orc, b):
-    n, w, h, c, k, bits = 4, 264, 40, 3, 5, 11
+@pytest.mark.parametrize("w,h,k,bits", [(264, 40, 5, 11), (320, 40, 3, 8)])   # thread-per-group kernels; tile kernels
+def test_packed_batch_equals_singles(orc, b, w, h, k, bits):
+    n, c = 4, 3
     key, nonce = synth.key_nonce(37)
     batch = b.PackedBatch(n, w, h, c, k, bits)
     nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
