@@ -177,15 +177,26 @@ __global__ void __launch_bounds__(PACKED_THREADS) packed_private_leaves_kernel(c
     const unsigned nblocks = (nbytes + 9u + 63u) / 64u;
     uint32_t H[8], w[16];
     sha256_init(H);
+    // message words from aligned 32-bit loads joined by a funnel shift; never past the last whole word of the image's fragment
+    const uintptr_t addr = reinterpret_cast<uintptr_t>(msg);
+    const uint32_t *aligned = reinterpret_cast<const uint32_t *>(addr & ~(uintptr_t)3);
+    const unsigned shift = 8u * (unsigned)(addr & 3u);
+    const uintptr_t safe_end = reinterpret_cast<uintptr_t>(p.priv + (size_t)n * p.priv_stride) + ((size_t)channels * p.nbr * p.packed_row_bytes & ~(size_t)3);
 #pragma unroll 1
     for (unsigned b = 0; b < nblocks; ++b) {
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
+            const unsigned pos0 = 64u * b + 4u * j;
             uint32_t word = 0u;
+            if (pos0 + 4u <= nbytes && addr + pos0 + 4u <= safe_end) {
+                const uint32_t lo = __ldg(aligned + (pos0 >> 2)), hi = shift ? __ldg(aligned + (pos0 >> 2) + 1) : 0u;
+                word = bswap32(__funnelshift_r(lo, hi, shift));
+            } else {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const unsigned pos = 64u * b + 4u * j + q;
-                word = (word << 8) | (pos < nbytes ? (uint32_t)msg[pos] : (pos == nbytes ? 0x80u : 0u));
+                for (int q = 0; q < 4; ++q) {
+                    const unsigned pos = pos0 + q;
+                    word = (word << 8) | (pos < nbytes ? (uint32_t)msg[pos] : (pos == nbytes ? 0x80u : 0u));
+                }
             }
             w[j] = word;
         }
