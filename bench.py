@@ -633,8 +633,11 @@ def main():
         alu_peak = 148 * 64 * sm_max_mhz * 1e6   # lane-ops/s
         aes_bound = alu_peak / (250.0 / 16.0) / 1e9     # 250 ALU-pipe ops per 16-byte block
         sha_bound = alu_peak / (1040.0 * 33 / 2048.0) / 1e9   # 33 compressions of 1040 ALU-pipe ops per 2048-byte leaf
+        # 160 table lookups per block, each a conflict-free 128-byte shared-memory wavefront, one per clock and SM: the tighter bound
+        lds_bound = 148 * sm_max_mhz * 1e6 / 160.0 * 32 * 16 / 1e9
         stages["aes128_ctr_stream"] = {"bytes": src.numel(), "GBps": src.numel() / (a_ms * 1e-3) / 1e9, "alu_bound_GBps": aes_bound,
                                        "frac_of_alu_bound": src.numel() / (a_ms * 1e-3) / 1e9 / aes_bound,
+                                       "lds_bound_GBps": lds_bound, "frac_of_lds_bound": src.numel() / (a_ms * 1e-3) / 1e9 / lds_bound,
                                        "note": "out-of-place over the whole input: the report's full-image AES baseline"}
         stages["sha256_merkle_stream"] = {"bytes": src.numel(), "GBps": src.numel() / (s_ms * 1e-3) / 1e9, "alu_bound_GBps": sha_bound,
                                           "frac_of_alu_bound": src.numel() / (s_ms * 1e-3) / 1e9 / sha_bound}
