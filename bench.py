@@ -368,7 +368,10 @@ def main():
                 B.profile_events(None, None)
     else:
         d_img = synth.image_batch_torch(1, w, h, c, seed=4000 + rank, device=dev)[0].contiguous()
-        ws = torch.empty(B.workspace_bytes(w, h, c, kl, True), dtype=torch.uint8, device=dev)
+        d_nonces = torch.from_numpy(sharding.nonces_for(nonce, rank, 1, priv_bytes=B.dwt_private_bytes(w, h, c, kl))).to(dev)
+        batch = B.DwtBatch(1, w, h, c, kl, device=dev)
+        d_rec = torch.empty_like(d_img)
+        aux = torch.cuda.Stream(device=dev)   # feds_defragment_dwt_batch_2s: verification on a second stream, joined before the call's end
         state = {}
 
         def step(record=False):
@@ -378,7 +381,7 @@ def main():
                 prof_frag.append((e0, e1))
                 call_frag.append((a, b_))
                 a.record()
-            pv, pb, dg = B.fragment_dwt(d_img, kl, key, nonce, workspace=ws)
+            batch.fragment(d_img, key, d_nonces)
             if record:
                 b_.record()
                 e2, e3, a2, b2 = ev(), ev(), ev(), ev()
@@ -386,11 +389,11 @@ def main():
                 prof_defrag.append((e2, e3))
                 call_defrag.append((a2, b2))
                 a2.record()
-            rec, fl = B.defragment_dwt(pv, pb, w, h, c, kl, key, nonce, expected=dg, workspace=ws)
+            batch.defragment_2s(d_rec, key, d_nonces, batch.digests, aux)
             if record:
                 b2.record()
                 B.profile_events(None, None)
-            state["rec"], state["fl"] = rec, fl
+            state["rec"], state["fl"] = d_rec, batch.flags_out
 
     def barrier():
         if world > 1:
@@ -745,7 +748,9 @@ def main():
                        "width": w, "height": h, "channels": c, "k_or_levels": kl,
                        "l2": "inputs+outputs per step (%.1f GB) exceed the 126 MB L2; no flush needed" % ((step_image_bytes * 10) / 1e9)
                        if step_image_bytes * 10 > 4e8 else "working set fits L2: cached numbers, reported as latency",
-                       "parallelism": "replicas (batch split), no collective"},
+                       "parallelism": "replicas (batch split), no collective",
+                       "calls": "feds_fragment_dct_batch + feds_defragment_dct_batch" if kind == "dct" else
+                                "feds_fragment_dwt_batch + feds_defragment_dwt_batch_2s (verification on a second stream, joined inside the call)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": gpu_launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "stages": stages,
         }

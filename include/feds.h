@@ -27,8 +27,10 @@ extern "C" {
 #if defined(__CUDACC__) || defined(__CUDA_RUNTIME_API_H__) || defined(__DRIVER_TYPES_H__)
 #include <cuda_runtime_api.h>
 typedef cudaStream_t feds_stream_t;
+typedef cudaEvent_t feds_event_t;
 #else
 typedef struct CUstream_st *feds_stream_t; /* identical to cudaStream_t */
+typedef struct CUevent_st *feds_event_t;   /* identical to cudaEvent_t */
 #endif
 
 typedef enum {
@@ -211,6 +213,24 @@ feds_status feds_defragment_dwt_batch(const uint8_t *d_private, size_t private_s
                                       const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
                                       uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
                                       feds_stream_t stream);
+
+/*
+ * feds_defragment_dwt_batch with the verification on a second stream. Recomputing the digests of the received fragments (leaf
+ * hashing, tree, compare: A10 "recompute + compare before use") and rebuilding the image from them (AES-CTR, inverse levels) read
+ * the same bytes and write disjoint parts of the workspace; on a single image the first is a chain of dependent hash launches
+ * that leaves the chip half empty and the second is bound by memory. This form enqueues the verification on aux_stream and the
+ * reconstruction on stream: fork_event is recorded on stream and waited for by aux_stream before its first kernel, join_event
+ * is recorded on aux_stream after the compare kernel and waited for by stream after the last level -- work enqueued on stream
+ * after the call sees both the image and the flags; nothing synchronises with the host; both streams may be under capture into
+ * one CUDA graph. The caller owns both streams and both events (any flags; cudaEventDisableTiming recommended) and must not
+ * reuse the events before the call's work has completed. d_expected_digests and d_verify_flags must not be NULL (without
+ * verification there is nothing to overlap: use feds_defragment_dwt_batch). Same results as feds_defragment_dwt_batch.
+ */
+feds_status feds_defragment_dwt_batch_2s(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                         int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *d_nonces,
+                                         const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                         uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                         feds_stream_t stream, feds_stream_t aux_stream, feds_event_t fork_event, feds_event_t join_event);
 
 /*
  * Batched DCT entry points ("series of images"): n_images images of identical shape, image i at

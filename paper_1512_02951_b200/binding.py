@@ -28,6 +28,7 @@ SYMBOLS = [
     "feds_workspace_bytes",
     "feds_fragment_dct", "feds_defragment_dct", "feds_fragment_dwt", "feds_defragment_dwt",
     "feds_fragment_dct_batch", "feds_defragment_dct_batch", "feds_fragment_dwt_batch", "feds_defragment_dwt_batch",
+    "feds_defragment_dwt_batch_2s",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
     "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
@@ -90,6 +91,8 @@ def _load():
     lib.feds_fragment_dct_packed_batch.argtypes = [vp, i, sz, i, i, i, i, i, u8p, vp, vp, sz, vp, sz, vp, vp, sz, vp]
     lib.feds_defragment_dct_packed_batch.argtypes = [vp, sz, vp, sz, i, i, i, i, i, i, u8p, vp, vp, vp, sz, vp, vp, sz, vp]
     lib.feds_defragment_dwt_batch.argtypes = lib.feds_defragment_dct_batch.argtypes
+    lib.feds_defragment_dwt_batch_2s.argtypes = list(lib.feds_defragment_dct_batch.argtypes) + [vp, vp, vp]
+    lib.feds_defragment_dwt_batch_2s.restype = i
     lib.feds_fragment_dct_host_scratch_bytes.restype = sz
     lib.feds_fragment_dct_host_scratch_bytes.argtypes = [i, i, i, i, i, i]
     lib.feds_fragment_dct_host.argtypes = [vp, i, i, i, i, i, u8p, vp, vp, vp, vp, i, vp, sz, C.POINTER(vp), i, C.c_uint]
@@ -522,6 +525,19 @@ class DwtBatch:
                                              self.c, self.levels, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
                                              self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
                                              _stream(stream)), "feds_defragment_dwt_batch")
+
+    def defragment_2s(self, images_out, key, d_nonces, expected, aux_stream, flags=FLAG_NONE, stream=None):
+        """feds_defragment_dwt_batch_2s: verification on aux_stream (a torch.cuda.Stream), reconstruction on `stream`"""
+        if not hasattr(self, "_events"):
+            self._events = [torch.cuda.Event(), torch.cuda.Event()]
+            for e in self._events:
+                e.record()   # torch creates the cudaEvent_t at the first record
+        fork, join = (C.c_void_p(e.cuda_event) for e in self._events)
+        _check(lib.feds_defragment_dwt_batch_2s(_ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, self.n, self.w, self.h,
+                                                self.c, self.levels, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
+                                                self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,
+                                                _stream(stream), C.c_void_p(aux_stream.cuda_stream), fork, join),
+               "feds_defragment_dwt_batch_2s")
 
 
 def fragment_dct_host(h_images, w, h, c, k, key, h_nonces, h_priv, h_pub, h_digests, images_per_chunk, d_scratch, streams,

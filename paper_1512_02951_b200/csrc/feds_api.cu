@@ -400,12 +400,14 @@ feds_status fragment_dwt_impl(const uint8_t *d_images, int n_images, size_t imag
 feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
                                 int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *nonce_host,
                                 const uint8_t *d_nonces, const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
-                                uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream) {
+                                uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags, cudaStream_t stream,
+                                cudaStream_t aux_stream = nullptr, cudaEvent_t fork_event = nullptr, cudaEvent_t join_event = nullptr) {
     feds_status st = check_dwt_args(n_images, w, h, c, levels);
     if (st != FEDS_OK) return st;
     if (flags & ~FEDS_FLAG_DWT_TILED) return FEDS_ERR_BAD_PARAM;
     if (!d_private || !d_public || !key || (!nonce_host && !d_nonces) || !d_images_out || !d_workspace || (d_expected_digests && !d_verify_flags))
         return FEDS_ERR_NULL_POINTER;
+    const bool two_streams = fork_event != nullptr;   // verification on aux_stream (feds_defragment_dwt_batch_2s)
     const DwtPlan pl = dwt_plan(w, h, c, levels);
     if (image_stride < (size_t)w * h * c || private_stride < pl.priv_b || public_stride < pl.pub_b) return FEDS_ERR_BAD_PARAM;
     if (misaligned(d_images_out) || misaligned(d_private) || misaligned(d_public) || misaligned(d_expected_digests) || misaligned(d_workspace) ||
@@ -417,18 +419,30 @@ feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride,
     const bool tiled = (flags & FEDS_FLAG_DWT_TILED) != 0;
 
     if (d_expected_digests) {
+        cudaStream_t vs = stream;
+        if (two_streams) {
+            FEDS_CUDA(cudaEventRecord(fork_event, stream));
+            FEDS_CUDA(cudaStreamWaitEvent(aux_stream, fork_event, 0));
+            vs = aux_stream;
+        }
         uint8_t *roots = ws + pl.per_image * (size_t)n_images - 64 * (size_t)n_images;
-        st = dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, ws + pl.planes_bytes * (size_t)n_images, roots, stream);
-        if (st != FEDS_OK) return st;
-        st = launch_compare_digests(roots, d_expected_digests, d_verify_flags, n_images, stream);
-        if (st != FEDS_OK) return st;
+        st = dwt_digests(d_private, private_stride, d_public, public_stride, n_images, pl, ws + pl.planes_bytes * (size_t)n_images, roots, vs);
+        if (st == FEDS_OK) st = launch_compare_digests(roots, d_expected_digests, d_verify_flags, n_images, vs);
+        if (two_streams) FEDS_CUDA(cudaEventRecord(join_event, aux_stream));
     }
+    // the reconstruction runs on `stream` meanwhile; `stream` waits for the verification at the very end (also after a failed
+    // launch: a capture must not be left forked)
+    auto joined = [&](feds_status s) {
+        if (two_streams && cudaStreamWaitEvent(stream, join_event, 0) != cudaSuccess && s == FEDS_OK) return FEDS_ERR_CUDA;
+        return s;
+    };
+    if (st != FEDS_OK) return joined(st);
     // decrypt LL_L into the level-L plane block (the received fragment stays untouched)
     // (image stride rounded up to 16 bytes: the CTR kernel moves 128-bit words; the plane block has 256-byte slack per image)
     uint8_t *lldec = ws + dwt_plane_off(pl, L, n_images);
     const size_t lldec_stride = round_up(pl.priv_b, 16);
     st = launch_aes_ctr(d_private, private_stride, lldec, lldec_stride, pl.priv_b, (unsigned)n_images, key, nonce_host, d_nonces, stream);
-    if (st != FEDS_OK) return st;
+    if (st != FEDS_OK) return joined(st);
 
     for (int l = L; l >= 1; --l) {
         DwtLevelParams p{};
@@ -444,9 +458,9 @@ feds_status defragment_dwt_impl(const uint8_t *d_private, size_t private_stride,
         p.img_out = d_images_out;
         if (l > 1) { p.ll_out_plane = reinterpret_cast<int16_t *>(ws + dwt_plane_off(pl, l - 1, n_images)); p.ll_out_plane_stride = (size_t)p.cw * p.ch; }
         st = launch_dwt_inv_level(p, l == 1, c, n_images, tiled, stream);
-        if (st != FEDS_OK) return st;
+        if (st != FEDS_OK) return joined(st);
     }
-    return FEDS_OK;
+    return joined(FEDS_OK);
 }
 
 // ---------------------------------------------------------------------------------------------- packed integer storage
@@ -852,6 +866,20 @@ feds_status feds_defragment_dwt_batch(const uint8_t *d_private, size_t private_s
     if (!d_nonces) return check_dwt_args(n_images, w, h, c, levels) != FEDS_OK ? check_dwt_args(n_images, w, h, c, levels) : FEDS_ERR_NULL_POINTER;
     return defragment_dwt_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, levels, key, nullptr, d_nonces,
                                d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, flags, stream);
+}
+
+feds_status feds_defragment_dwt_batch_2s(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
+                                         int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *d_nonces,
+                                         const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
+                                         uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
+                                         feds_stream_t stream, feds_stream_t aux_stream, feds_event_t fork_event, feds_event_t join_event) {
+    const feds_status st = check_dwt_args(n_images, w, h, c, levels);
+    if (st != FEDS_OK) return st;
+    if (!d_nonces || !d_expected_digests || !d_verify_flags || !aux_stream || !fork_event || !join_event) return FEDS_ERR_NULL_POINTER;
+    if (aux_stream == stream) return FEDS_ERR_BAD_PARAM;
+    return defragment_dwt_impl(d_private, private_stride, d_public, public_stride, n_images, w, h, c, levels, key, nullptr, d_nonces,
+                               d_expected_digests, d_images_out, image_stride, d_verify_flags, d_workspace, workspace_bytes, flags, stream,
+                               aux_stream, fork_event, join_event);
 }
 
 feds_status feds_verify_dwt(const uint8_t *d_private, const uint8_t *d_public, int w, int h, int c, int levels,

@@ -119,3 +119,43 @@ def test_dwt_batch_equals_oracle_per_image(orc, b, n, w, h, c, L):
     want[victim] |= 2
     want[0] |= 1
     assert batch.flags_out.cpu().tolist() == want
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,w,h,c,L", [(1, 1024, 512, 1, 3), (3, 256, 128, 3, 2)])
+def test_two_stream_defragment_equals_single_stream(orc, b, n, w, h, c, L):
+    """feds_defragment_dwt_batch_2s (verification on a second stream, joined at the end): the image and the flags are those of the
+    single-stream call, which the tests above pin to the oracle -- also after tampering, also when the pair of streams is captured
+    into one CUDA graph and replayed."""
+    key, nonce = synth.key_nonce(5 * w + n)
+    imgs = np.stack([synth.image(w, h, c, seed=70 * w + i, rectangles=2) for i in range(n)])
+    batch = b.DwtBatch(n, w, h, c, L)
+    nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
+    d_imgs, d_non = torch.from_numpy(imgs).cuda(), torch.from_numpy(nonces).cuda()
+    batch.fragment(d_imgs, key, d_non)
+    aux = torch.cuda.Stream()
+    out = torch.zeros_like(d_imgs)
+    batch.flags_out.fill_(9)
+    batch.defragment_2s(out, key, d_non, batch.digests, aux)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and batch.flags_out.cpu().tolist() == [0] * n
+    # capture both streams into one graph (the first call above set the kernel attributes), replay on tampered fragments
+    main = torch.cuda.Stream()
+    main.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=main):
+        batch.defragment_2s(out, key, d_non, batch.digests, aux, stream=main)
+    batch.pub[(n - 1) * batch.pub_stride + 11] ^= 0x40
+    batch.priv[5] ^= 1
+    want = [0] * n
+    want[n - 1] |= 2
+    want[0] |= 1
+    ref_out = torch.zeros_like(d_imgs)
+    batch.defragment(ref_out, key, d_non, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert batch.flags_out.cpu().tolist() == want
+    for _ in range(3):
+        out.zero_(); batch.flags_out.fill_(9)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref_out) and batch.flags_out.cpu().tolist() == want

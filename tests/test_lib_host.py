@@ -65,6 +65,16 @@ def test_argument_errors_are_reported_before_any_launch(b):
     assert g(ok_ptr, 16, 16, 1, 0, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 1 << 20, None) == 3
     assert g(ok_ptr, 64, 64, 1, 2, key, key, ok_ptr, ok_ptr, ok_ptr, ok_ptr, 8, None) == 4
     assert b.lib.feds_status_string(2) == b"bad dimensions"
+    # two-stream verified defragment: needs digests, flags, a second stream (not the call's own) and both events
+    t = b.lib.feds_defragment_dwt_batch_2s
+    args = [ok_ptr, 4096, ok_ptr, 4096, 1, 64, 64, 1, 2, key, ok_ptr, ok_ptr, ok_ptr, 4096, ok_ptr, ok_ptr, 1 << 20, 0]
+    assert t(*args, ok_ptr, None, ok_ptr, ok_ptr) == 1                      # no aux stream
+    assert t(*args, ok_ptr, C.c_void_p(0x2000), None, ok_ptr) == 1           # no fork event
+    assert t(*args, ok_ptr, ok_ptr, ok_ptr, ok_ptr) == 3                     # aux stream == stream
+    no_digests = list(args); no_digests[11] = None
+    assert t(*no_digests, ok_ptr, C.c_void_p(0x2000), ok_ptr, ok_ptr) == 1   # nothing to verify: use feds_defragment_dwt_batch
+    bad = list(args); bad[5] = 62
+    assert t(*bad, ok_ptr, C.c_void_p(0x2000), ok_ptr, ok_ptr) == 2          # bad dims come first
 
 
 def test_binding_has_no_cpu_fallback():
