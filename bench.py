@@ -227,6 +227,7 @@ def sweep_arm(args, desc):
     key, nonce = synth.key_nonce(5)
     points = []
     sizes = [256, 512, 1024, 2048, 4096, 8192, 16384]
+    aux = torch.cuda.Stream(device=dev)   # DWT points: verified defragment with its hash chain on a second stream (feds_defragment_dwt_batch_2s)
     if args.images > 0:
         sizes = [x for x in sizes if x <= args.images]   # --images N caps the edge length (quick runs)
     for sz in sizes:
@@ -256,13 +257,13 @@ def sweep_arm(args, desc):
                            "hbm_frac": nbytes * 10 / ms / 1e6 / hbm_peak})
             del batch
         for L in [1, 2, 3, 4]:
-            ws = torch.empty(B.workspace_bytes(sz, sz, 3, L, True), dtype=torch.uint8, device=dev)
             im = img[0]
-            st = {}
+            db = B.DwtBatch(1, sz, sz, 3, L, device=dev)
+            st = {"rec": torch.empty_like(im), "fl": db.flags_out}
 
             def one():
-                pv, pb, dg = B.fragment_dwt(im, L, key, nonce, workspace=ws)
-                st["rec"], st["fl"] = B.defragment_dwt(pv, pb, sz, sz, 3, L, key, nonce, expected=dg, workspace=ws)
+                db.fragment(im, key, d_non)
+                db.defragment_2s(st["rec"], key, d_non, db.digests, aux)
             for _ in range(3):
                 one()
             torch.cuda.synchronize()
@@ -276,7 +277,7 @@ def sweep_arm(args, desc):
             ms = e0.elapsed_time(e1) / reps
             points.append({"path": "dwt", "size": sz, "levels": L, "ms": ms, "MBps": nbytes / ms / 1e3, "hbm_GBps": nbytes * 6 / ms / 1e6,
                            "hbm_frac": nbytes * 6 / ms / 1e6 / hbm_peak})
-            del ws, st
+            del db, st
         del img, out
         torch.cuda.empty_cache()
     big = [p_ for p_ in points if p_["path"] == "dct" and p_["size"] == sizes[-1]]

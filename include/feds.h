@@ -225,13 +225,14 @@ feds_status feds_defragment_dwt_batch(const uint8_t *d_private, size_t private_s
  * one CUDA graph. The caller owns both streams and both events (any flags; cudaEventDisableTiming recommended) and must not
  * reuse the events before the call's work has completed. d_expected_digests and d_verify_flags must not be NULL (without
  * verification there is nothing to overlap: use feds_defragment_dwt_batch). Same results as feds_defragment_dwt_batch.
+ * (There is no such form for the DCT path: its reconstruction kernel is one persistent CTA per SM, and sharing the chip with
+ * the hash kernel leaves some of those CTAs without an SM until the hashing is over -- measured: up to 1.9x slower at 2048^2.)
  */
 feds_status feds_defragment_dwt_batch_2s(const uint8_t *d_private, size_t private_stride, const uint8_t *d_public, size_t public_stride,
                                          int n_images, int w, int h, int c, int levels, const uint8_t key[16], const uint8_t *d_nonces,
                                          const uint8_t *d_expected_digests, uint8_t *d_images_out, size_t image_stride,
                                          uint32_t *d_verify_flags, void *d_workspace, size_t workspace_bytes, unsigned flags,
                                          feds_stream_t stream, feds_stream_t aux_stream, feds_event_t fork_event, feds_event_t join_event);
-
 /*
  * Batched DCT entry points ("series of images"): n_images images of identical shape, image i at
  * d_images + i*image_stride, fragments at d_private + i*private_stride / d_public + i*public_stride, digests at

@@ -142,6 +142,15 @@ def _stream(stream):
     return C.c_void_p(s.cuda_stream)
 
 
+def _fork_join_events(owner):
+    """the two cudaEvent_t a *_2s call needs, created once per batch object (torch creates the event at its first record)"""
+    if not hasattr(owner, "_events"):
+        owner._events = [torch.cuda.Event(), torch.cuda.Event()]
+        for e in owner._events:
+            e.record()
+    return tuple(C.c_void_p(e.cuda_event) for e in owner._events)
+
+
 def _k16(b):
     """key / nonce: exactly 16 bytes (the library reads 16 bytes from the pointer it is given)."""
     b = bytes(b)
@@ -528,11 +537,7 @@ class DwtBatch:
 
     def defragment_2s(self, images_out, key, d_nonces, expected, aux_stream, flags=FLAG_NONE, stream=None):
         """feds_defragment_dwt_batch_2s: verification on aux_stream (a torch.cuda.Stream), reconstruction on `stream`"""
-        if not hasattr(self, "_events"):
-            self._events = [torch.cuda.Event(), torch.cuda.Event()]
-            for e in self._events:
-                e.record()   # torch creates the cudaEvent_t at the first record
-        fork, join = (C.c_void_p(e.cuda_event) for e in self._events)
+        fork, join = _fork_join_events(self)
         _check(lib.feds_defragment_dwt_batch_2s(_ptr(self.priv), self.priv_stride, _ptr(self.pub), self.pub_stride, self.n, self.w, self.h,
                                                 self.c, self.levels, _k16(key), _ptr(d_nonces), _ptr(expected), _ptr(images_out),
                                                 self.image_bytes, _ptr(self.flags_out), _ptr(self.ws), self.ws.numel(), flags,

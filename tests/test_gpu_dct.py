@@ -542,3 +542,4 @@ def test_cuda_graph_capture_and_replay(orc, b):
     assert (p2 == pv).all() and (q2 == pb).all() and d2 == dct.digests[:64].cpu().numpy().tobytes()
     op, oq, odg = orc.fragment_dwt(imgs[0][0].cpu().numpy(), L, key, nonces[0].tobytes())
     assert (dwt.priv[:dwt.priv_bytes].cpu().numpy() == op).all() and dwt.digests[:64].cpu().numpy().tobytes() == odg
+
