@@ -91,7 +91,9 @@ def test_streaming_and_tiled_level_kernels_agree(orc, b, w, h, c, L):
 
 
 @pytest.mark.parametrize("n,w,h,c,L", [(3, 64, 32, 1, 2), (4, 272, 144, 3, 3), (2, 1024, 320, 3, 4), (5, 16, 8, 1, 1), (3, 48, 80, 4, 2),
-                                       (2, 2048, 512, 1, 3)])
+                                       (2, 2048, 512, 1, 3),
+                                       # public trees of 1,536 / 2,304 leaves: the spread-out tree top with four and six trees in flight
+                                       (2, 2048, 1024, 1, 1), (3, 1024, 1024, 3, 2)])
 def test_dwt_batch_equals_oracle_per_image(orc, b, n, w, h, c, L):
     """feds_fragment_dwt_batch / feds_defragment_dwt_batch: every image is an independent CTR message with its own nonce and digest
     pair (A20); each image's fragments and digests are the oracle's, bit for bit; verification flags are per image."""
