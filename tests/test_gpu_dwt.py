@@ -64,8 +64,29 @@ def test_dwt_verify_flags(orc, b):
 
 
 def test_config4_full_size(orc, b):
-    """8192x8192 grayscale, 3 levels (BASELINE config 4): bit-exact on everything."""
-    run_case(orc, b, synth.image(8192, 8192, 1, seed=4), 3, seed=4)
+    """8192x8192 grayscale, 3 levels (BASELINE config 4): bit-exact on everything -- and once more through the calls and in the
+    launch configuration bench.py times (batch entry points, the verified defragment on two streams): fragments and digests are
+    the oracle's, the image comes back exactly, a flipped bit in either fragment raises its flag."""
+    img = synth.image(8192, 8192, 1, seed=4)
+    run_case(orc, b, img, 3, seed=4)
+    key, nonce = synth.key_nonce(4)
+    batch = b.DwtBatch(1, 8192, 8192, 1, 3)
+    d_img = torch.from_numpy(img).cuda()
+    d_non = torch.frombuffer(bytearray(nonce), dtype=torch.uint8).cuda().view(1, 16)
+    batch.fragment(d_img, key, d_non)
+    op, oq, odg = orc.fragment_dwt(img, 3, key, nonce)
+    assert (batch.priv[:batch.priv_bytes].cpu().numpy() == op).all() and (batch.pub[:batch.pub_bytes].cpu().numpy() == oq).all()
+    assert batch.digests.cpu().numpy().tobytes() == odg
+    aux, rec = torch.cuda.Stream(), torch.zeros_like(d_img)
+    batch.flags_out.fill_(9)
+    batch.defragment_2s(rec, key, d_non, batch.digests, aux)
+    torch.cuda.synchronize()
+    assert torch.equal(rec, d_img) and batch.flags_out.cpu().tolist() == [0]
+    batch.pub[batch.pub_bytes - 1] ^= 0x80
+    batch.priv[0] ^= 1
+    batch.defragment_2s(rec, key, d_non, batch.digests, aux)
+    torch.cuda.synchronize()
+    assert batch.flags_out.cpu().tolist() == [3]
 
 
 @pytest.mark.parametrize("w,h,c,L", [(1024, 320, 3, 4), (2048, 64, 1, 1), (7696, 96, 1, 2), (496, 80, 3, 1)])
