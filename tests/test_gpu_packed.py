@@ -130,3 +130,44 @@ def test_packed_full_hd_image_and_overheads(orc, b):
     for bits, frac in ((11, 11 * 6 / 64 / 8), (8, 5 / 64 + 11 / 8 / 64)):
         d_img, priv, pub, dg, key, nonce = check(orc, b, img, 5, bits, seed=8)
         assert priv.numel() / img.size == pytest.approx(frac, abs=1e-9)
+
+
+def test_packed_config3_batch_full_size(orc, b):
+    """BASELINE config 3 (256 x 1920x1080 RGB, k = 3) through the packed 11-bit storage, in the launch configuration bench.py
+    times (feds_*_dct_packed_batch, tile kernels with 148 persistent CTAs): every image comes back exactly with no flag raised;
+    a sample of images -- first, last and six in between -- goes through stages (i) and (ii) against the oracle on host threads."""
+    from concurrent.futures import ThreadPoolExecutor
+    n, w, h, c, k, bits = 256, 1920, 1080, 3, 3, 11
+    key, nonce = synth.key_nonce(33)
+    batch = b.PackedBatch(n, w, h, c, k, bits)
+    nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
+    d_non = torch.from_numpy(nonces).cuda()
+    d_imgs = synth.image_batch_torch(n, w, h, c, seed=3300, device="cuda", rectangles=8)
+    batch.fragment(d_imgs, key, d_non)
+    out = torch.zeros_like(d_imgs)
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    M = (1 << (bits - 1)) - 1
+
+    def one(i):
+        img = d_imgs[i].cpu().numpy()
+        pv = batch.priv[i * batch.priv_stride:i * batch.priv_stride + batch.priv_bytes].cpu().numpy()
+        pb = batch.pub[i * batch.pub_stride:i * batch.pub_stride + batch.pub_bytes].cpu().numpy()
+        q = gpu_integers(orc, pv, w, h, c, k, bits, key, nonces[i].tobytes())
+        ref = orc.dct_coefficients(img)[:, :k + 1].copy()
+        ref[:, 0] = np.clip(ref[:, 0], 0, 2047)
+        ref[:, 1:] = np.clip(ref[:, 1:], -M, M)
+        assert np.abs(q - ref).max() <= 0.5 + 1e-3, i
+        p2, q2, d2 = orc.fragment_packed_from_q(img, q, k, bits, key, nonces[i].tobytes())
+        assert (p2 == pv).all() and (q2 == pb).all() and d2 == batch.digests[64 * i:64 * i + 64].cpu().numpy().tobytes(), i
+        return i
+
+    sample = [0, 37, 74, 111, 148, 185, 222, 255]
+    with ThreadPoolExecutor(8) as ex:
+        assert sorted(ex.map(one, sample)) == sample
+    batch.pub[200 * batch.pub_stride + 77] ^= 1
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    want = [0] * n
+    want[200] = 2
+    assert batch.flags_out.cpu().tolist() == want
