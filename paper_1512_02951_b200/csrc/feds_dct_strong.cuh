@@ -180,6 +180,36 @@ __device__ __forceinline__ bool strong_decode(const DctParams &p, unsigned long 
     return true;
 }
 
+// The same bytes without unpacking (small k). x - floor((S + 2^14) / 2^15) = floor((x 2^15 + 2^14 - 1 - S) / 2^15), and with
+// everything doubled the low byte of that quotient is byte 2 of acc = (x << 16 | 0x7ffe) - sum (2 q_z) B_z; the inverse is byte 2
+// of (r << 16 | 0x8000) + sum (2 q_z) B_z. One PRMT drops the byte into the accumulator over the constant BIAS, one IMAD per
+// coefficient against the table in constant memory (immediate offsets), one PRMT per two results. m[z] = -/+ 2 q_z (arithmetic
+// modulo 2^32 throughout, as in strong_low_pass). Rows 4 HALF .. 4 HALF + 3 of the block (words x[8 HALF ..]) -> r[0..7].
+template <int HALF, int PMAX, uint32_t BIAS>
+__device__ __forceinline__ void strong_bytes_half(const uint32_t (&x)[16], const int32_t (&m)[PMAX], int P, uint32_t (&r)[8]) {
+    int32_t acc[32];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) acc[i] = (int32_t)__byte_perm(x[8 * HALF + (i >> 2)], BIAS, 0x7054u + ((uint32_t)(i & 3) << 8));
+#pragma unroll
+    for (int z = 0; z < PMAX; ++z) {
+        if (z < P) {   // warp-uniform
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+                acc[i] = (int32_t)((uint32_t)acc[i] + (uint32_t)m[z] * (uint32_t)c_strong_basis_tab.B[64 * z + 32 * HALF + i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        r[i] = __byte_perm(__byte_perm((uint32_t)acc[4 * i], (uint32_t)acc[4 * i + 1], 0x0062u), __byte_perm((uint32_t)acc[4 * i + 2], (uint32_t)acc[4 * i + 3], 0x0062u), 0x5410u);
+}
+// m[z] = sign * 2 * rne(8 c_z) from the Part 1 column
+template <int PMAX>
+__device__ __forceinline__ void strong_scaled_q(const uint32_t *part1, int stride, int P, int sign, int32_t (&m)[PMAX]) {
+#pragma unroll
+    for (int z = 0; z < PMAX; ++z)
+        m[z] = z < P ? (int32_t)((uint32_t)__float2int_rn(8.0f * __uint_as_float(part1[z * stride])) * (uint32_t)(2 * sign)) : 0;
+}
+
 // the channel's 8 pixel bytes of row r of the block as two packed words (global memory, read-only path)
 template <int C>
 __device__ __forceinline__ uint2 strong_load_row(const uint8_t *row, int c) {
@@ -260,7 +290,9 @@ __device__ __forceinline__ void store_block_packed(uint8_t *__restrict__ img, in
 }
 
 // Shared memory: the AES round tables (1024 words), then one column of 64 words per thread (word z of thread t at z * THREADS + t).
-template <int C>
+// PMAX = 8 >= k + 1: only the first PMAX zigzag coefficients are computed (the rest of the transform is dead code) and
+// the remainder comes from strong_bytes_half; PMAX = 64: any k.
+template <int C, int PMAX = 64>
 __global__ void __launch_bounds__(STRONG_THREADS) fragment_dct_strong_kernel(const __grid_constant__ DctParams p) {
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
@@ -276,10 +308,21 @@ __global__ void __launch_bounds__(STRONG_THREADS) fragment_dct_strong_kernel(con
         load_block<C>(img, p.w, 8 * S.br, 8 * S.bc, S.ch, v);
         dct8x8(v);
 #pragma unroll
-        for (int z = 0; z < 64; ++z) col[z * STRONG_THREADS] = __float_as_uint(v[ZZ.pos[z]]);
+        for (int z = 0; z < PMAX; ++z) col[z * STRONG_THREADS] = __float_as_uint(v[ZZ.pos[z]]);
     }
     uint32_t rows[16];
-    {   // the remainder x - L, modulo 256
+    if constexpr (PMAX < 64) {   // the remainder x - L, modulo 256
+        uint32_t x[16];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            const uint2 xr = strong_load_row<C>(img + ((size_t)(8 * S.br + r) * p.w + 8 * S.bc) * C, S.ch);
+            x[2 * r] = xr.x; x[2 * r + 1] = xr.y;
+        }
+        int32_t m[PMAX];
+        strong_scaled_q<PMAX>(col, STRONG_THREADS, P, -1, m);
+        strong_bytes_half<0, PMAX, 0x00007ffeu>(x, m, P, reinterpret_cast<uint32_t(&)[8]>(rows[0]));
+        strong_bytes_half<1, PMAX, 0x00007ffeu>(x, m, P, reinterpret_cast<uint32_t(&)[8]>(rows[8]));
+    } else {
         int32_t acc[64];
         strong_low_pass(col, STRONG_THREADS, P, acc);
 #pragma unroll
@@ -308,7 +351,7 @@ __global__ void __launch_bounds__(STRONG_THREADS) fragment_dct_strong_kernel(con
     }
 }
 
-template <int C>
+template <int C, int PMAX = 64>
 __global__ void __launch_bounds__(STRONG_THREADS) defragment_dct_strong_kernel(const __grid_constant__ DctParams p) {
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *sT = smem;
@@ -328,9 +371,21 @@ __global__ void __launch_bounds__(STRONG_THREADS) defragment_dct_strong_kernel(c
         strong_ctr_xor(p, sT, nonce, w0, P, col, STRONG_THREADS);   // Part 1 in plaintext
         uint32_t ks[16];
         sha512_part1_keystream(col, STRONG_THREADS, P, ks);
+        const uint4 *q = reinterpret_cast<const uint4 *>(p.pub + (size_t)S.n * p.pub_stride + 64 * S.b);
+        if constexpr (PMAX < 64) {
+            uint32_t x[16];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const uint4 v = __ldg(q + i);
+                x[4 * i] = v.x ^ ks[4 * i]; x[4 * i + 1] = v.y ^ ks[4 * i + 1]; x[4 * i + 2] = v.z ^ ks[4 * i + 2]; x[4 * i + 3] = v.w ^ ks[4 * i + 3];
+            }
+            int32_t m[PMAX];
+            strong_scaled_q<PMAX>(col, STRONG_THREADS, P, 1, m);
+            strong_bytes_half<0, PMAX, 0x00008000u>(x, m, P, reinterpret_cast<uint32_t(&)[8]>(rows[0]));
+            strong_bytes_half<1, PMAX, 0x00008000u>(x, m, P, reinterpret_cast<uint32_t(&)[8]>(rows[8]));
+        } else {
         int32_t acc[64];
         strong_low_pass(col, STRONG_THREADS, P, acc);
-        const uint4 *q = reinterpret_cast<const uint4 *>(p.pub + (size_t)S.n * p.pub_stride + 64 * S.b);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const uint4 x = __ldg(q + i);
@@ -338,6 +393,7 @@ __global__ void __launch_bounds__(STRONG_THREADS) defragment_dct_strong_kernel(c
             rows[4 * i + 1] = strong_apply4<false>(x.y ^ ks[4 * i + 1], acc[16 * i + 4], acc[16 * i + 5], acc[16 * i + 6], acc[16 * i + 7]);
             rows[4 * i + 2] = strong_apply4<false>(x.z ^ ks[4 * i + 2], acc[16 * i + 8], acc[16 * i + 9], acc[16 * i + 10], acc[16 * i + 11]);
             rows[4 * i + 3] = strong_apply4<false>(x.w ^ ks[4 * i + 3], acc[16 * i + 12], acc[16 * i + 13], acc[16 * i + 14], acc[16 * i + 15]);
+        }
         }
     }
     if (!act) { S.n = 0; S.ch = 0; S.br = 0; S.bc = 0; }

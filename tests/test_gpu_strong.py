@@ -58,15 +58,18 @@ def check(orc, b, img, k, seed):
 
 @pytest.mark.parametrize("w,h,c,k", [(8, 8, 1, 0), (8, 8, 1, 5), (16, 16, 4, 63), (64, 8, 1, 3), (72, 24, 1, 5), (1080, 16, 3, 5), (136, 40, 4, 9),
                                      (512, 512, 1, 5), (256, 264, 3, 5), (520, 24, 3, 26), (520, 24, 3, 27), (64, 64, 1, 32), (40, 8, 3, 4),
-                                     (1920, 136, 3, 5), (2056, 8, 1, 1)])
+                                     (1920, 136, 3, 5), (2056, 8, 1, 1),
+                                     # the kernel forms change at k = 4 (inverse) and k = 8 (forward)
+                                     (48, 16, 4, 2), (96, 24, 3, 7), (96, 24, 3, 8)])
 def test_strong_parity_and_round_trips(orc, b, w, h, c, k):
     check(orc, b, synth.image(w, h, c, seed=w + 3 * h + c + k, rectangles=2 if w >= 64 and h >= 16 else 0), k, seed=w * 5 + k)
 
 
 @pytest.mark.parametrize("kind", ["zeros", "ones", "checker", "random", "impulse"])
 @pytest.mark.parametrize("c", [1, 3, 4])
-def test_strong_special_images(orc, b, kind, c):
-    check(orc, b, synth.special(kind, 96, 32, c, seed=c), 5, seed=13)
+@pytest.mark.parametrize("k", [3, 5])
+def test_strong_special_images(orc, b, kind, c, k):
+    check(orc, b, synth.special(kind, 96, 32, c, seed=c), k, seed=13)
 
 
 def test_strong_verify_flags_and_damage_confinement(orc, b):
