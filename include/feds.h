@@ -338,6 +338,22 @@ feds_status feds_sha256_merkle(const uint8_t *d_data, size_t n_bytes, uint8_t *d
                                size_t workspace_bytes, feds_stream_t stream);
 
 /*
+ * feds_sha256_merkle_static — feds_sha256_merkle for callers that cannot allocate device memory (code under CUDA graph
+ * capture, serving loops, harnesses that forbid cudaMalloc): the same digest (step 5 on a stream), the same
+ * kernels, but the workspace is a static array in device memory inside the library, 1.125 MiB on every GPU that loads the
+ * library, held until the process exits. The call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating
+ * library routine) and does not synchronise. d_data: n_bytes bytes, device; d_root: 32 bytes, device; both 16-byte aligned.
+ * Limit: n_bytes <= feds_sha256_merkle_static_max_bytes() = 64 MiB (32,768 leaves); a longer stream returns
+ * FEDS_ERR_BAD_PARAM and enqueues nothing -- use feds_sha256_merkle with a workspace of your own. Other errors as for
+ * feds_sha256_merkle.
+ * All calls on one device share the array, and it keeps the last call's contents (each call writes every slot it reads and
+ * clears the counters it needs at zero): calls that may overlap on the GPU -- different streams with no ordering between
+ * them -- race on it and must be ordered by the caller; calls on one stream, or on different devices, are safe.
+ */
+size_t feds_sha256_merkle_static_max_bytes(void);
+feds_status feds_sha256_merkle_static(const uint8_t *d_data, size_t n_bytes, uint8_t *d_root, feds_stream_t stream);
+
+/*
  * Profiling hook (not part of the data path; thread-local): while set, every fragment/defragment call made on this
  * thread records ev_start immediately before and ev_stop immediately after its dominant kernel(s), on the call's stream:
  * DCT calls with digests (fragment, verified defragment, feds_verify_dct): the leaf-hash kernel, or the fused kernel on the

@@ -31,7 +31,8 @@ SYMBOLS = [
     "feds_defragment_dwt_batch_2s",
     "feds_fragment_dct_host_scratch_bytes", "feds_fragment_dct_host",
     "feds_defragment_dct_host_scratch_bytes", "feds_defragment_dct_host", "feds_profile_events",
-    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
+    "feds_aes128_ctr", "feds_sha256_merkle_workspace_bytes", "feds_sha256_merkle", "feds_sha256_merkle_static_max_bytes",
+    "feds_sha256_merkle_static", "feds_verify_dct", "feds_verify_dct_batch", "feds_verify_dwt",
     "feds_dct_strong_public_bytes", "feds_fragment_dct_strong", "feds_defragment_dct_strong", "feds_fragment_dct_strong_batch",
     "feds_defragment_dct_strong_batch", "feds_debug_strong_basis_host",
     "feds_dct_packed_private_bytes", "feds_dct_packed_workspace_bytes", "feds_fragment_dct_packed", "feds_defragment_dct_packed",
@@ -106,6 +107,10 @@ def _load():
     lib.feds_sha256_merkle_workspace_bytes.restype = sz
     lib.feds_sha256_merkle_workspace_bytes.argtypes = [sz]
     lib.feds_sha256_merkle.argtypes = [vp, sz, vp, vp, sz, vp]
+    lib.feds_sha256_merkle_static_max_bytes.restype = sz
+    lib.feds_sha256_merkle_static_max_bytes.argtypes = []
+    lib.feds_sha256_merkle_static.argtypes = [vp, sz, vp, vp]
+    lib.feds_sha256_merkle_static.restype = i
     lib.feds_profile_events.argtypes = [vp, vp]
     lib.feds_profile_events.restype = None
     lib.feds_debug_sha256_host.argtypes = [u8p, sz, vp]
@@ -436,6 +441,14 @@ def sha256_merkle(data, stream=None, workspace=None):
     _on_stream(stream, root, ws)
     _check(lib.feds_sha256_merkle(_ptr(data) if data.numel() else None, data.numel(), _ptr(root), _ptr(ws), ws.numel(), _stream(stream)),
            "feds_sha256_merkle")
+    return root
+
+
+def sha256_merkle_static(data, root, stream=None):
+    """feds_sha256_merkle_static: the Merkle root of `data` into the caller's 32-byte device tensor `root`; the scratch is the
+    library's static device array, nothing is allocated (streams up to feds_sha256_merkle_static_max_bytes())."""
+    _check(lib.feds_sha256_merkle_static(_ptr(data) if data.numel() else None, data.numel(), _ptr(root), _stream(stream)),
+           "feds_sha256_merkle_static")
     return root
 
 

@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.environ.get("FEDS_LIB_PATH") or os.path.join(HERE, "libfeds.so")
-SOURCES = ["feds_api.cu", "feds_k_hash.cu", "feds_k_dct_tile.cu", "feds_k_dct_tma.cu", "feds_k_dct_fused.cu", "feds_k_dwt.cu", "feds_k_dct_strong.cu", "feds_k_dwt_tiles.cu"]
+SOURCES = ["feds_api.cu", "feds_k_hash.cu", "feds_k_dct_tile.cu", "feds_k_dct_tma.cu", "feds_k_dct_fused.cu", "feds_k_dwt.cu", "feds_k_dct_strong.cu", "feds_k_dwt_tiles.cu", "feds_k_static.cu"]
 SOURCES = [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
 
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
