@@ -713,6 +713,7 @@ def main():
         h_pb = torch.empty(pbb, dtype=torch.uint8).pin_memory()
         h_dg = torch.empty(64, dtype=torch.uint8).pin_memory()
         d_in = torch.empty_like(d_img)
+        ws = torch.empty(B.workspace_bytes(w, h, c, kl, True), dtype=torch.uint8, device=dev)
 
         def e2e_step():
             d_in.copy_(h_img, non_blocking=True)
