@@ -123,3 +123,43 @@ def test_strong_batch_equals_singles(orc, b):
 def test_strong_full_hd_image(orc, b):
     """one 1920x1080 RGB image, k = 5 (the report's default selection): stage (ii) on the whole image, exact round trip"""
     check(orc, b, synth.image(1920, 1080, 3, seed=8, rectangles=8), 5, seed=8)
+
+
+@pytest.mark.parametrize("k", [3, 5])
+def test_strong_config3_batch_full_size(orc, b, k):
+    """BASELINE config 3 (256 x 1920x1080 RGB) through the strong level in the launch configuration bench.py times
+    (feds_*_dct_strong_batch; k = 3 is bench.py's stage, k = 5 the report's default selection and the other forward kernel form):
+    every image comes back exactly with no flag raised; eight images -- first, last, six in between -- go through stages (i) and
+    (ii) against the oracle on host threads; a flipped public byte raises exactly its image's flag."""
+    from concurrent.futures import ThreadPoolExecutor
+    n, w, h, c = 256, 1920, 1080, 3
+    key, nonce = synth.key_nonce(40 + k)
+    batch = b.StrongBatch(n, w, h, c, k)
+    nonces = synth.batch_nonces(nonce, n, priv_bytes=batch.priv_bytes)
+    d_non = torch.from_numpy(nonces).cuda()
+    d_imgs = synth.image_batch_torch(n, w, h, c, seed=4400 + k, device="cuda", rectangles=8)
+    batch.fragment(d_imgs, key, d_non)
+    out = torch.zeros_like(d_imgs)
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_imgs) and int(batch.flags_out.abs().sum().item()) == 0
+    nb, P = c * (h // 8) * (w // 8), k + 1
+
+    def one(i):
+        img = d_imgs[i].cpu().numpy()
+        pv = batch.priv[i * batch.priv_stride:i * batch.priv_stride + batch.priv_bytes].cpu().numpy()
+        pb = batch.pub[i * batch.pub_stride:i * batch.pub_stride + batch.pub_bytes].cpu().numpy()
+        part1 = np.frombuffer(orc.aes128_ctr_xor(key, nonces[i].tobytes(), pv.tobytes()), dtype="<f4").reshape(nb, P)
+        assert np.abs(part1.astype(np.float64) - orc.dct_coefficients(img)[:, :P]).max() <= TOL, i
+        p2, q2, d2 = orc.fragment_strong_from_priv32(img, part1, k, key, nonces[i].tobytes())
+        assert (p2 == pv).all() and (q2 == pb).all() and d2 == batch.digests[64 * i:64 * i + 64].cpu().numpy().tobytes(), i
+        return i
+
+    sample = [0, 37, 74, 111, 148, 185, 222, 255]
+    with ThreadPoolExecutor(8) as ex:
+        assert sorted(ex.map(one, sample)) == sample
+    batch.pub[100 * batch.pub_stride + 12345] ^= 4
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    want = [0] * n
+    want[100] = 2
+    assert batch.flags_out.cpu().tolist() == want
