@@ -100,3 +100,27 @@ def test_tiles_batch_equals_oracle_per_image(orc, b):
     batch.pub[1 * batch.pub_stride + 9] ^= 4
     batch.defragment(out, key, d_non, expected=batch.digests)
     assert batch.flags_out.cpu().tolist() == [0, 2, 0]
+
+
+def test_tiles_config4_full_size(orc, b):
+    """8192 x 8192 gray (BASELINE config 4) through the batch entry points bench.py times for this design: both fragments and the
+    digests are the oracle's, bit for bit; the image comes back exactly; a flipped bit in either fragment raises its flag."""
+    w = h = 8192
+    img = synth.image(w, h, 1, seed=44)
+    key, nonce = synth.key_nonce(44)
+    batch = b.TilesBatch(1, w, h, 1)
+    d_img = torch.from_numpy(img).cuda()
+    d_non = torch.frombuffer(bytearray(nonce), dtype=torch.uint8).cuda().view(1, 16)
+    batch.fragment(d_img, key, d_non)
+    torch.cuda.synchronize()
+    op, oq, odg = orc.fragment_tiled(img, key, nonce)
+    assert (batch.priv[:batch.priv_bytes].cpu().numpy() == op).all() and (batch.pub[:batch.pub_bytes].cpu().numpy() == oq).all()
+    assert batch.digests.cpu().numpy().tobytes() == odg
+    out = torch.zeros_like(d_img)
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    torch.cuda.synchronize()
+    assert torch.equal(out, d_img) and batch.flags_out.cpu().tolist() == [0]
+    batch.pub[batch.pub_bytes - 1] ^= 0x80
+    batch.priv[0] ^= 1
+    batch.defragment(out, key, d_non, expected=batch.digests)
+    assert batch.flags_out.cpu().tolist() == [3]
