@@ -244,7 +244,7 @@ feds_status defragment_dct_impl(const uint8_t *d_private, size_t private_stride,
     if (verify) {
         p.leaves = verification_leaves(pl, n_images, static_cast<uint8_t *>(d_workspace));
         // Verification and reconstruction read the same fragments. Fused route: one warp-specialised kernel whose hash warps
-        // and reconstruction warps walk the leaves together, so the fragments come from HBM once (feds_dct_ws.cuh). Split
+        // and reconstruction warps walk the leaves together, so the fragments come from HBM once (feds_dct_fused.cuh; forced route only). Split
         // route: the registers-only leaf-hash kernel, then the digest-free tile kernel.
         const Route route = pick_route(p, c, flags);
         if (route == Route::Unsupported) return FEDS_ERR_BAD_PARAM;

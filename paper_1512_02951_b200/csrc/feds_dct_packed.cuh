@@ -4,7 +4,8 @@
 // AES-128-CTR; the public part is the image-sized remainder x - L ("IDCT of the rest"), taken against the QUANTISED Part 1 in
 // the fixed-point arithmetic of the strong level, so that every pixel comes back exactly with either storage.
 //
-// One thread per (leaf group, channel): it walks the group's blocks, appends their fields to a bit buffer and writes the group's
+// These are the general kernels (any shape, any k); feds_dct_packed_tile.cuh has the tile-group kernels the host prefers where the
+// shape allows (w % 64 == 0, k <= 15). One thread per (leaf group, channel): it walks the group's blocks, appends their fields to a bit buffer and writes the group's
 // bytes. The channels of one pixel strip sit in adjacent lanes (store_block_packed). Encryption is the stream kernel's, in place.
 #pragma once
 #include "feds_dct_strong.cuh"

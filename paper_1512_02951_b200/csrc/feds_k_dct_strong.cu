@@ -1,5 +1,5 @@
 // feds_k_dct_strong.cu — launchers of the strong-level kernels (feds_dct_strong.cuh; PAPER.md 6.3.2) and of the packed-storage kernels
-// (feds_dct_packed.cuh; PAPER.md 6.4.3), which share the fixed-point basis table.
+// (feds_dct_packed.cuh and, on bulk-copy tile groups, feds_dct_packed_tile.cuh; PAPER.md 6.4.3), which share the fixed-point basis table.
 #include <algorithm>
 
 #include "feds_dct_packed_tile.cuh"
