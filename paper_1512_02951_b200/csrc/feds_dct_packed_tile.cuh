@@ -161,7 +161,7 @@ __device__ __forceinline__ void packed_fragment_block(const DctParams &p, const 
     packed_remainder_half<1, PMAX>(x, q, P, dst);
 }
 
-// PMAX (4, 8 or 16) >= k + 1: the unrolled per-coefficient code the kernel carries
+// PMAX (4, 6, 8 or 16) >= k + 1: the unrolled per-coefficient code the kernel carries
 template <int C, int PMAX>
 __global__ void __launch_bounds__(PackedTileShape<C>::CTA, 1) fragment_dct_packed_tile_kernel(const __grid_constant__ DctParams p) {
     using S = TmaShape<C>;

@@ -71,7 +71,7 @@ bool packed_tile_supported(const DctParams &p, int c) {
 feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t stream, bool profile) {
     if (packed_tile_supported(p, c)) {
 #define FEDS_PT(CC, PM) { static size_t set = 0; return launch_packed_tile<CC>(fragment_dct_packed_tile_kernel<CC, PM>, set, p, stream, profile); }
-#define FEDS_PT_P(CC) { if (p.k < 4) FEDS_PT(CC, 4) else if (p.k < 8) FEDS_PT(CC, 8) else FEDS_PT(CC, 16) }
+#define FEDS_PT_P(CC) { if (p.k < 4) FEDS_PT(CC, 4) else if (p.k < 6) FEDS_PT(CC, 6) else if (p.k < 8) FEDS_PT(CC, 8) else FEDS_PT(CC, 16) }
         if (c == 1) FEDS_PT_P(1) else if (c == 3) FEDS_PT_P(3) else FEDS_PT_P(4)
 #undef FEDS_PT_P
 #undef FEDS_PT
@@ -90,7 +90,7 @@ feds_status launch_fragment_packed(const DctParams &p, int c, cudaStream_t strea
 feds_status launch_defragment_packed(const DctParams &p, int c, const uint8_t *plain, size_t plain_stride, cudaStream_t stream, bool profile) {
     if (packed_tile_supported(p, c)) {
 #define FEDS_PT(CC, PM) { static size_t set = 0; return launch_packed_tile<CC>(defragment_dct_packed_tile_kernel<CC, PM>, set, p, stream, profile, plain, plain_stride); }
-#define FEDS_PT_P(CC) { if (p.k < 4) FEDS_PT(CC, 4) else if (p.k < 8) FEDS_PT(CC, 8) else FEDS_PT(CC, 16) }
+#define FEDS_PT_P(CC) { if (p.k < 4) FEDS_PT(CC, 4) else if (p.k < 6) FEDS_PT(CC, 6) else if (p.k < 8) FEDS_PT(CC, 8) else FEDS_PT(CC, 16) }
         if (c == 1) FEDS_PT_P(1) else if (c == 3) FEDS_PT_P(3) else FEDS_PT_P(4)
 #undef FEDS_PT_P
 #undef FEDS_PT
