@@ -290,7 +290,7 @@ __device__ __forceinline__ void store_block_packed(uint8_t *__restrict__ img, in
 }
 
 // Shared memory: the AES round tables (1024 words), then one column of 64 words per thread (word z of thread t at z * THREADS + t).
-// PMAX = 8 >= k + 1: only the first PMAX zigzag coefficients are computed (the rest of the transform is dead code) and
+// PMAX = 4 or 8 >= k + 1: only the first PMAX zigzag coefficients are computed (the rest of the transform is dead code) and
 // the remainder comes from strong_bytes_half; PMAX = 64: any k.
 template <int C, int PMAX = 64>
 __global__ void __launch_bounds__(STRONG_THREADS) fragment_dct_strong_kernel(const __grid_constant__ DctParams p) {

@@ -21,7 +21,8 @@ feds_status launch_fragment_strong(const DctParams &p, int c, cudaStream_t strea
     const unsigned grid = (unsigned)((threads + STRONG_THREADS - 1) / STRONG_THREADS);
     if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
     // measured on the cfg3 batch: the pruned-transform form wins up to k = 7 (k = 3: 8.12 -> 7.37 ms, k = 5: 8.89 -> 8.14), is level at k = 9
-#define FEDS_S(CC) { if (p.k < 8) fragment_dct_strong_kernel<CC, 8><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); \
+#define FEDS_S(CC) { if (p.k < 4) fragment_dct_strong_kernel<CC, 4><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); \
+                     else if (p.k < 8) fragment_dct_strong_kernel<CC, 8><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); \
                      else fragment_dct_strong_kernel<CC, 64><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); }
     if (c == 1) FEDS_S(1) else if (c == 3) FEDS_S(3) else FEDS_S(4)
 #undef FEDS_S
@@ -35,7 +36,7 @@ feds_status launch_defragment_strong(const DctParams &p, int c, cudaStream_t str
     const unsigned grid = (unsigned)((threads + STRONG_THREADS - 1) / STRONG_THREADS);
     if (prof_start_event() && profile) FEDS_CUDA(cudaEventRecord(prof_start_event(), stream));
     // the inverse has no transform to prune: the unrolled accumulators win only for k <= 3 (7.58 -> 7.37 ms; k = 5: 8.37 -> 8.58)
-#define FEDS_S(CC) { if (p.k < 4) defragment_dct_strong_kernel<CC, 8><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); \
+#define FEDS_S(CC) { if (p.k < 4) defragment_dct_strong_kernel<CC, 4><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); \
                      else defragment_dct_strong_kernel<CC, 64><<<grid, STRONG_THREADS, STRONG_SMEM, stream>>>(p); }
     if (c == 1) FEDS_S(1) else if (c == 3) FEDS_S(3) else FEDS_S(4)
 #undef FEDS_S
