@@ -46,7 +46,7 @@ def test_static_scratch_root_equals_workspace_path_on_consecutive_calls(orc, b):
         b.sha256_merkle_static(data, root)
         b.sha256_merkle_static(data, root)                 # twice in a row on the same stream: same scratch, same answer
         torch.cuda.synchronize()
-        assert torch.cuda.memory_allocated() == before     # the binding marshals arguments only
+        assert torch.cuda.memory_allocated() <= before     # the binding marshals arguments only (the count may drop: garbage of earlier tests)
         assert torch.equal(root, want), (i, n)
         if n <= (3 << 20):
             assert root.cpu().numpy().tobytes() == orc.merkle_stream(data.cpu().numpy().tobytes()), (i, n)
